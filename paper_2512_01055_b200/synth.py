@@ -1,0 +1,207 @@
+"""Seeded synthetic inputs for the closed-shell (T) energy.
+
+This module is shared by the oracle's tests and by the CUDA path's tests and
+bench.  It holds NO arithmetic of the (T) method itself: it only draws the
+problem inputs (DF factors, orbital energies, amplitudes) and derives the
+integral blocks the boundary accepts.  It imports neither ``oracle`` nor the
+CUDA binding.
+
+Recipe (BASELINE.json ``configs``):
+
+* ``B^Q_pq ~ N(0, sigma_B^2)`` (sigma_B = 0.05), drawn for ``p <= q`` and
+  mirrored, ``p, q`` over ``o+v`` orbitals with the occupied ones first, so
+  that ``(pq|rs) = sum_Q B^Q_pq B^Q_rs`` exactly (eq. (6)).
+* ``eps_occ ~ U[-2.0, -0.3]``, ``eps_vir ~ U[0.1, 5.0]``.
+* ``t2`` = MP2 amplitudes ``(ia|jb) / (e_i + e_j - e_a - e_b)``, symmetrised
+  bit-exactly so that ``t_ij^ab == t_ji^ba``.
+* ``t1 ~ N(0, 0.01^2)``.
+
+Random numbers come from a counter-based generator (splitmix64 of
+``(seed, tensor id, flat index)`` then Box-Muller), so every element of every
+tensor is a pure function of its index.
+
+A second, closed-form input family (``closed_form_problem``) reproduces the
+worked examples of SURVEY.md section 8(c) P10.
+"""
+from __future__ import annotations
+
+import dataclasses
+from typing import Optional
+
+import numpy as np
+
+_M64 = np.uint64(0xFFFFFFFFFFFFFFFF)
+_GOLD = 0x9E3779B97F4A7C15
+_MIX1 = 0xBF58476D1CE4E5B9
+_MIX2 = 0x94D049BB133111EB
+
+TENSOR_B = 1
+TENSOR_EPS_OCC = 2
+TENSOR_EPS_VIR = 3
+TENSOR_T1 = 4
+
+# BASELINE.json configs[0..4]: (o, v, naux, seed)
+CONFIGS = {
+    "cfg0": (8, 40, 120, 0),
+    "cfg1": (20, 200, 600, 1),
+    "cfg2": (40, 400, 1200, 2),
+    "cfg3": (60, 500, 1500, 3),
+    "cfg4": (100, 800, 2400, 4),
+}
+
+
+def _splitmix64(x: np.ndarray) -> np.ndarray:
+    """One splitmix64 output for each 64-bit state in ``x`` (uint64 array)."""
+    with np.errstate(over="ignore"):
+        z = x + np.uint64(_GOLD)
+        z = (z ^ (z >> np.uint64(30))) * np.uint64(_MIX1)
+        z = (z ^ (z >> np.uint64(27))) * np.uint64(_MIX2)
+        z = z ^ (z >> np.uint64(31))
+    return z
+
+
+def _uniform_pair(seed: int, tensor_id: int, idx: np.ndarray):
+    """Two uniforms per counter: u1 in (0, 1], u2 in [0, 1)."""
+    idx = np.asarray(idx, dtype=np.uint64)
+    with np.errstate(over="ignore"):
+        base = (np.uint64((seed * _GOLD) & 0xFFFFFFFFFFFFFFFF)
+                ^ np.uint64((tensor_id * _MIX1) & 0xFFFFFFFFFFFFFFFF))
+        ctr = base + np.uint64(2) * idx
+        r1 = _splitmix64(ctr)
+        r2 = _splitmix64(ctr + np.uint64(1))
+    scale = 1.0 / 9007199254740992.0  # 2^-53
+    u1 = ((r1 >> np.uint64(11)).astype(np.float64) + 1.0) * scale
+    u2 = (r2 >> np.uint64(11)).astype(np.float64) * scale
+    return u1, u2
+
+
+def counter_normal(seed: int, tensor_id: int, idx, sigma: float) -> np.ndarray:
+    u1, u2 = _uniform_pair(seed, tensor_id, idx)
+    return sigma * np.sqrt(-2.0 * np.log(u1)) * np.cos(2.0 * np.pi * u2)
+
+
+def counter_uniform(seed: int, tensor_id: int, idx, lo: float, hi: float) -> np.ndarray:
+    _, u2 = _uniform_pair(seed, tensor_id, idx)
+    return lo + (hi - lo) * u2
+
+
+@dataclasses.dataclass
+class Problem:
+    """Inputs of one (T) calculation, all float64, C order (host numpy arrays).
+
+    Layouts are those of include/tc_triples.h:
+      Boo[Q][i][j], Bov[Q][i][a], Bvv[Q][a][b];
+      t1[i][a]; t2[i][j][a][b] = t_ij^ab;
+      vvvo[x][d][b][c] = (bd|cx); ovoo[j][k][l][c] = (lj|kc); ovov[j][k][b][c] = (jb|kc).
+    The integral blocks are optional (None until ``materialise_blocks``).
+    """
+    o: int
+    v: int
+    naux: int
+    eps_occ: np.ndarray
+    eps_vir: np.ndarray
+    t1: np.ndarray
+    t2: np.ndarray
+    Boo: np.ndarray
+    Bov: np.ndarray
+    Bvv: np.ndarray
+    vvvo: Optional[np.ndarray] = None
+    ovoo: Optional[np.ndarray] = None
+    ovov: Optional[np.ndarray] = None
+
+
+def _split_B(B: np.ndarray, o: int):
+    Boo = np.ascontiguousarray(B[:, :o, :o])
+    Bov = np.ascontiguousarray(B[:, :o, o:])
+    Bvv = np.ascontiguousarray(B[:, o:, o:])
+    return Boo, Bov, Bvv
+
+
+def mp2_amplitudes(Bov: np.ndarray, eps_occ: np.ndarray, eps_vir: np.ndarray) -> np.ndarray:
+    """t2[i][j][a][b] = (ia|jb) / (e_i + e_j - e_a - e_b), made exactly symmetric
+    under (i,a) <-> (j,b) by averaging with its own transpose."""
+    naux, o, v = Bov.shape
+    M = Bov.reshape(naux, o * v)
+    iajb = (M.T @ M).reshape(o, v, o, v)              # (ia|jb)
+    den = (eps_occ[:, None, None, None] - eps_vir[None, :, None, None]
+           + eps_occ[None, None, :, None] - eps_vir[None, None, None, :])
+    t = iajb / den                                    # [i][a][j][b]
+    t = 0.5 * (t + t.transpose(2, 3, 0, 1))           # bit-exact t_ij^ab = t_ji^ba
+    return np.ascontiguousarray(t.transpose(0, 2, 1, 3))   # [i][j][a][b]
+
+
+def make_problem(o: int, v: int, naux: int, seed: int, sigma_B: float = 0.05,
+                 sigma_t1: float = 0.01, blocks: bool = False) -> Problem:
+    """Draw one synthetic problem with the BASELINE.json recipe."""
+    N = o + v
+    p = np.arange(N, dtype=np.uint64)
+    lo = np.minimum(p[:, None], p[None, :])
+    hi = np.maximum(p[:, None], p[None, :])
+    pair = lo * np.uint64(N) + hi                    # (min, max) -> mirrored draw
+    B = np.empty((naux, N, N), dtype=np.float64)
+    for Q in range(naux):
+        idx = np.uint64(Q) * np.uint64(N * N) + pair
+        B[Q] = counter_normal(seed, TENSOR_B, idx, sigma_B)
+    eps_occ = counter_uniform(seed, TENSOR_EPS_OCC, np.arange(o), -2.0, -0.3)
+    eps_vir = counter_uniform(seed, TENSOR_EPS_VIR, np.arange(v), 0.1, 5.0)
+    t1 = counter_normal(seed, TENSOR_T1, np.arange(o * v), sigma_t1).reshape(o, v)
+    Boo, Bov, Bvv = _split_B(B, o)
+    t2 = mp2_amplitudes(Bov, eps_occ, eps_vir)
+    prob = Problem(o, v, naux, eps_occ, eps_vir, np.ascontiguousarray(t1), t2, Boo, Bov, Bvv)
+    if blocks:
+        materialise_blocks(prob)
+    return prob
+
+
+def make_config(name: str, blocks: bool = False, sigma_B: float = 0.05) -> Problem:
+    o, v, naux, seed = CONFIGS[name]
+    return make_problem(o, v, naux, seed, sigma_B=sigma_B, blocks=blocks)
+
+
+def closed_form_problem(o: int, v: int, naux: int, blocks: bool = True,
+                        t1_zero: bool = False) -> Problem:
+    """Closed-form inputs of the worked examples:
+    B^Q_pq = 0.3 cos(0.7(Q+1) + 1.3(p+q) + 0.11 p q) / (1 + 0.1|p-q|),
+    eps_occ[i] = -1.5 + 0.35 i, eps_vir[a] = 0.4 + 0.45 a,
+    t1[i][a] = 0.02 sin(1 + 2i + 3a), t2 = MP2 from B."""
+    N = o + v
+    Q = np.arange(naux, dtype=np.float64)[:, None, None]
+    p = np.arange(N, dtype=np.float64)[None, :, None]
+    q = np.arange(N, dtype=np.float64)[None, None, :]
+    B = 0.3 * np.cos(0.7 * (Q + 1.0) + 1.3 * (p + q) + 0.11 * p * q) / (1.0 + 0.1 * np.abs(p - q))
+    eps_occ = -1.5 + 0.35 * np.arange(o, dtype=np.float64)
+    eps_vir = 0.4 + 0.45 * np.arange(v, dtype=np.float64)
+    ii = np.arange(o, dtype=np.float64)[:, None]
+    aa = np.arange(v, dtype=np.float64)[None, :]
+    t1 = 0.02 * np.sin(1.0 + 2.0 * ii + 3.0 * aa)
+    if t1_zero:
+        t1 = np.zeros_like(t1)
+    Boo, Bov, Bvv = _split_B(B, o)
+    t2 = mp2_amplitudes(Bov, eps_occ, eps_vir)
+    prob = Problem(o, v, naux, eps_occ, eps_vir, np.ascontiguousarray(t1), t2, Boo, Bov, Bvv)
+    if blocks:
+        materialise_blocks(prob)
+    return prob
+
+
+def vvvo_slice(prob: Problem, x: int) -> np.ndarray:
+    """I_x[d][b][c] = (bd|cx) for one occupied index x (v^3 doubles)."""
+    naux, v = prob.naux, prob.v
+    A = prob.Bvv.reshape(naux, v * v)                 # [Q][(d,b)] (Bvv is symmetric)
+    return (A.T @ prob.Bov[:, x, :]).reshape(v, v, v)
+
+
+def materialise_blocks(prob: Problem) -> Problem:
+    """Fill vvvo / ovoo / ovov from the DF factors (input preparation only)."""
+    o, v, naux = prob.o, prob.v, prob.naux
+    vvvo = np.empty((o, v, v, v), dtype=np.float64)
+    for x in range(o):
+        vvvo[x] = vvvo_slice(prob, x)
+    # ovoo[j][k][l][c] = (lj|kc) = sum_Q Boo[Q][l][j] Bov[Q][k][c]
+    ovoo = np.einsum("qlj,qkc->jklc", prob.Boo, prob.Bov, optimize=True)
+    # ovov[j][k][b][c] = (jb|kc) = sum_Q Bov[Q][j][b] Bov[Q][k][c]
+    ovov = np.einsum("qjb,qkc->jkbc", prob.Bov, prob.Bov, optimize=True)
+    prob.vvvo = vvvo
+    prob.ovoo = np.ascontiguousarray(ovoo)
+    prob.ovov = np.ascontiguousarray(ovov)
+    return prob
