@@ -1,0 +1,180 @@
+/*
+ * tc_triples.h -- C-ABI of the B200-native closed-shell (T) energy library.
+ *
+ * What it computes (arxiv 2512.01055, "Accelerating CCSD(T) on GPUs"; citations are
+ * PAPER.md line numbers):
+ *
+ *   E(T) = sum_{i>=j>=k} (2 - d_ij - d_jk) S_ijk                        eq. (1)
+ *   S_ijk = sum_abc (W_abc + Vd_abc) R_abc / D_abc                      (virtual-index form of eq. (1))
+ *   W_ijk^abc = P [ sum_d t_ij^ad (bd|ck) - sum_l t_il^ab (lj|kc) ]     eqs. (2),(5)
+ *   Vd_ijk^abc = t_i^a (jb|kc) + t_j^b (ia|kc) + t_k^c (ia|jb)          eq. (3)
+ *   D_ijk^abc = e_i + e_j + e_k - e_a - e_b - e_c                       Fig. 4 l.23
+ *   R_abc = 4W_abc + W_bca + W_cab - 2W_acb - 2W_cba - 2W_bac           eq. (1) weights
+ *   (pq|rs) = sum_Q B^Q_pq B^Q_rs                                       eq. (6)
+ *
+ * All arithmetic is FP64 and runs in hand-written sm_100a kernels; there is no CPU
+ * fallback: on a machine without a compute-capability-10.x device every compute call
+ * returns TC_ERR_UNSUPPORTED_DEVICE.
+ *
+ * Conventions common to all calls
+ *   - No exceptions cross the boundary; every call returns a tc_status.  On error the
+ *     output arguments are untouched and tc_last_error(ctx) describes the failure.
+ *   - "device" pointers are CUDA device memory on the context's device, owned by the
+ *     caller, read-only to the library unless stated, and must stay valid until the
+ *     call returns.  "host" pointers are ordinary host memory.
+ *   - All arrays are FP64 ("double"), dense, C order (last index fastest).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Work is enqueued on it; side streams the library owns are forked from and joined
+ *     to it with events, so the caller sees single-stream semantics.  Calls that
+ *     return a host scalar synchronise `stream` once before returning.
+ *   - The library performs no device allocation inside the compute calls: scratch
+ *     space is the caller-allocated `workspace` (the paper's "pre-allocate and reuse"
+ *     rule).  tc_workspace_bytes tells how much is needed.
+ *
+ * Triplet linear index (defines "a contiguous slice of triplets"):
+ *   idx(i,j,k) = i(i+1)(i+2)/6 + j(j+1)/2 + k   for i >= j >= k >= 0.
+ */
+#ifndef TC_TRIPLES_H
+#define TC_TRIPLES_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TC_OK = 0,
+    TC_ERR_INVALID_ARG = 1,
+    TC_ERR_UNSUPPORTED_DEVICE = 2,
+    TC_ERR_WORKSPACE_TOO_SMALL = 3,
+    TC_ERR_CUDA = 4,
+    TC_ERR_INTERNAL = 5
+} tc_status;
+
+typedef struct tc_ctx tc_ctx; /* opaque; owns streams/events and a few KB of pinned memory */
+
+/* Materialised integral blocks (device pointers). */
+typedef struct {
+    const double* vvvo; /* [x][d][b][c] = (bd|cx), o*v^3; slice x is contiguous (the paper's (vv|vo) block) */
+    const double* ovoo; /* [j][k][l][c] = (lj|kc), o^3*v */
+    const double* ovov; /* [j][k][b][c] = (jb|kc), o^2*v^2 */
+} tc_int_blocks;
+
+/* Density-fitting (or Cholesky, eq. (6)) factors (device pointers). */
+typedef struct {
+    int naux;
+    const double* Boo; /* [Q][i][j] */
+    const double* Bov; /* [Q][i][a] */
+    const double* Bvv; /* [Q][a][b], symmetric in a,b */
+} tc_df_factors;
+
+/* ---- context ------------------------------------------------------------------- */
+
+/* Create a context on CUDA device `device`.  Fails with TC_ERR_UNSUPPORTED_DEVICE if
+ * there is no such device or its compute capability is not 10.x. */
+tc_status tc_create(tc_ctx** ctx, int device);
+tc_status tc_destroy(tc_ctx* ctx);
+const char* tc_status_string(tc_status s);
+const char* tc_last_error(const tc_ctx* ctx); /* never NULL; valid until the next call on ctx */
+
+/* ---- a1: triplet scheduler (host, no GPU needed) -------------------------------- */
+
+/* o(o+1)(o+2)/6, or -1 if o < 1. */
+long long tc_triplet_count(int o);
+/* idx -> (i,j,k) and the degeneracy weight 2 - d_ij - d_jk (0 for i=j=k). */
+tc_status tc_triplet_decode(int o, long long idx, int* i, int* j, int* k, double* weight);
+/* (i,j,k), i>=j>=k -> idx, or -1 if the arguments are not an ordered triplet below o. */
+long long tc_triplet_index(int o, int i, int j, int k);
+
+/* ---- workspace ------------------------------------------------------------------ */
+
+/* Bytes of device workspace tc_triples_energy / _slice need for a problem of this size.
+ *   naux_or_0   : naux when DF factors will be passed, 0 when integral blocks are passed.
+ *   hbm_budget  : upper bound the caller is willing to give (0 = no bound).  With DF
+ *                 input the library materialises all (vv|vo) slices if they fit in the
+ *                 budget, else it sizes an LRU cache of per-occupied-index slices.
+ * Returns TC_ERR_WORKSPACE_TOO_SMALL if even the minimum does not fit the budget. */
+tc_status tc_workspace_bytes(tc_ctx* ctx, int o, int v, int naux_or_0, size_t hbm_budget, size_t* bytes);
+
+/* ---- a2: integral staging from DF factors --------------------------------------- */
+
+/* Assemble integral blocks on the device from DF factors with the library's FP64
+ * tensor-core GEMM (eq. (6)).  Each output pointer may be NULL (skipped):
+ *   vvvo_out [x0 <= x < x0+nx][d][b][c] (nx*v^3), ovoo_out (o^3 v), ovov_out (o^2 v^2).
+ * Asynchronous on `stream`. */
+tc_status tc_build_blocks(tc_ctx* ctx, int o, int v, const tc_df_factors* df,
+                          int x0, int nx, double* vvvo_out, double* ovoo_out, double* ovov_out,
+                          void* stream);
+
+/* ---- a3-a7: the (T) energy ------------------------------------------------------ */
+
+/* E(T) over all triplets.  Exactly one of `blocks` / `df` is non-NULL.
+ *   eps_occ[o], eps_vir[v], t1[i][a], t2[i][j][a][b] (= t_ij^ab; precondition
+ *   t_ij^ab == t_ji^ba): device.  E_out: host.  */
+tc_status tc_triples_energy(tc_ctx* ctx, int o, int v,
+                            const double* eps_occ, const double* eps_vir,
+                            const double* t1, const double* t2,
+                            const tc_int_blocks* blocks, const tc_df_factors* df,
+                            void* workspace, size_t workspace_bytes,
+                            void* stream, double* E_out);
+
+/* The same over triplets first .. first+count-1 of the linear index.
+ *   S_dev (device, [count], optional): receives S_ijk of each triplet (0 for i=j=k).
+ *   E_partial_out (host): sum of weight * S_ijk over the range. */
+tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v,
+                                  const double* eps_occ, const double* eps_vir,
+                                  const double* t1, const double* t2,
+                                  const tc_int_blocks* blocks, const tc_df_factors* df,
+                                  void* workspace, size_t workspace_bytes,
+                                  void* stream, long long first, long long count,
+                                  double* S_dev, double* E_partial_out);
+
+/* End-to-end variant with HOST inputs: copies the DF factors, amplitudes and orbital
+ * energies to the device (cudaMalloc/cudaFree inside; this is the one call that
+ * allocates), assembles the integrals, computes E(T), returns it on the host.
+ * If bytes_h2d != NULL it receives the bytes copied host->device. */
+tc_status tc_triples_energy_host(tc_ctx* ctx, int o, int v, int naux,
+                                 const double* eps_occ, const double* eps_vir,
+                                 const double* t1, const double* t2,
+                                 const double* Boo, const double* Bov, const double* Bvv,
+                                 long long first, long long count,
+                                 double* E_out, size_t* bytes_h2d);
+
+/* Debug/validation: W_ijk^abc (eqs. (2),(5)) of one triplet written to W_dev[a][b][c]
+ * (device, v^3) by the same tile kernels that feed the fused epilogue.  Any order of
+ * i,j,k is accepted.  Used by the parity tests only. */
+tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j, int k,
+                             const double* t2, const tc_int_blocks* blocks,
+                             double* W_dev, void* stream);
+
+/* ---- statistics of the last energy call ----------------------------------------- */
+
+typedef struct {
+    long long n_triplets;        /* triplets in the range with non-zero weight          */
+    long long n_work_units;      /* (triplet, virtual tile orbit) units executed         */
+    long long n_kernel_launches; /* kernels this library launched during the call        */
+    double    flop_contraction;  /* executed o^3v^4 + o^4v^3 contraction flop (useful)   */
+    double    ms_total;          /* device time of the whole call (CUDA events)          */
+    double    ms_contraction;    /* device time of the fused W-builder kernels           */
+    double    ms_staging;        /* device time of DF->block assembly (0 with blocks)    */
+    long long slices_built;      /* (vv|v.) slices assembled from DF during the call     */
+} tc_stats;
+tc_status tc_get_stats(const tc_ctx* ctx, tc_stats* out);
+
+/* ---- microbenchmarks: the roofline denominators ---------------------------------- */
+
+/* Register-resident FP64 tensor-core (mma.sync m8n8k4 f64 -> DMMA.8x8x4) throughput.
+ * Runs for about `seconds`; returns sustained TFLOP/s and the best single-launch
+ * (burst) TFLOP/s. */
+tc_status tc_bench_dmma_peak(tc_ctx* ctx, double seconds, double* tflops_sustained, double* tflops_burst);
+/* The same with scalar FP64 FMA (DFMA). */
+tc_status tc_bench_dfma_peak(tc_ctx* ctx, double seconds, double* tflops_sustained, double* tflops_burst);
+/* Device copy bandwidth (read+write bytes / time), GB/s, over `bytes` per direction
+ * of caller-provided device buffers. */
+tc_status tc_bench_copy_bw(tc_ctx* ctx, void* dst_dev, const void* src_dev, size_t bytes, int reps, double* gbs);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TC_TRIPLES_H */

@@ -1,0 +1,112 @@
+// tc_common.cuh -- shared declarations of the (T) library's translation units.
+// Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/tc_triples.h"
+
+struct tc_ctx {
+    int device;
+    int sm_count;
+    int cc_major, cc_minor;
+    size_t smem_optin;
+    size_t l2_bytes;
+    cudaStream_t side_stream;      // integral staging runs here (a2)
+    cudaEvent_t ev_fork, ev_join;  // fork/join of side_stream against the caller's stream
+    cudaEvent_t ev_t0, ev_t1, ev_s0, ev_s1, ev_c0, ev_c1;
+    double* pinned;                // a few doubles of pinned host memory for scalar results
+    tc_stats stats;
+    char err[512];
+};
+
+#define TC_FAIL(ctx, code, ...)                                        \
+    do {                                                               \
+        if (ctx) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__); \
+        return (code);                                                 \
+    } while (0)
+
+#define TC_CUDA(ctx, call)                                                                  \
+    do {                                                                                    \
+        cudaError_t e__ = (call);                                                           \
+        if (e__ != cudaSuccess)                                                             \
+            TC_FAIL(ctx, TC_ERR_CUDA, "%s:%d: %s -> %s", __FILE__, __LINE__, #call,         \
+                    cudaGetErrorString(e__));                                               \
+    } while (0)
+
+// ---- FP64 tensor-core primitive -------------------------------------------------------
+// mma.sync m8n8k4 f64: the only FP64 MMA shape that is a single native instruction on
+// sm_100a (SASS DMMA.8x8x4).  Fragment layout (PTX ISA):
+//   A[row = lane>>2][k = lane&3], B[k = lane&3][col = lane>>2],
+//   C[row = lane>>2][col = 2*(lane&3) + {0,1}].
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+// ---- cp.async helpers (LDGSTS) --------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+// 16-byte copy, src_bytes in [0,16] valid bytes, the rest zero-filled.
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes));
+}
+// 8-byte copy, src_bytes in {0,8}.
+__device__ __forceinline__ void cp_async8(uint32_t dst, const void* src, int src_bytes) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
+
+// ---- internal entry points (defined in the other .cu files) ---------------------------
+
+// a2: C = A^T B with K-major operands and a 2-level output index map (tc_stager.cu).
+//   A[K][M], B[K][N] (leading dimensions lda, ldb), row = r1*R2 + r2, col = c1*C2 + c2,
+//   C[r1*sr1 + r2*sr2 + c1*sc1 + c2*sc2] = sum_k A[k][row] B[k][col].
+cudaError_t tc_launch_df_gemm(const double* A, size_t lda, const double* B, size_t ldb, int M, int N, int K,
+                              int R2, long long sr1, long long sr2, int C2, long long sc1, long long sc2,
+                              double* C, cudaStream_t stream);
+
+// a3-a6: fused W-builder + epilogue over a range of triplets (tc_wbuild.cu).
+struct tc_wbuild_args {
+    int o, v;
+    const double* eps_occ;
+    const double* eps_vir;
+    const double* t1;
+    const double* t2;
+    const double* const* slice_ptr;  // device array [o]: slice_ptr[x] -> I_x[d][b][c] (NULL if not resident)
+    bool slices_aligned16;           // every resident slice starts on a 16-byte boundary
+    const double* ovoo;
+    const double* ovov;
+    const int4* triplets;            // device array [n_trip]: (i, j, k, row of partial[])
+    int n_trip;
+    double* partial;                 // device [n_trip][n_orbits] per-unit partial sums
+    int n_orbits;
+    double* W_debug;                 // optional v^3 output of W for n_trip == 1
+};
+size_t tc_wbuild_smem_bytes();
+int tc_wbuild_tile();                                  // virtual tile edge T
+int tc_wbuild_num_orbits(int v);                       // nb(nb+1)(nb+2)/6
+cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const int4* orbits /*device [n_orbits]: (A,B,C,0), A>=B>=C*/,
+                             cudaStream_t stream);
+
+// a7: deterministic reductions (tc_reduce.cu).
+//   triplets[t] = decode(first + t) as (i, j, k, t); w[t] = 2 - d_ij - d_jk
+cudaError_t tc_launch_make_triplets(int o, long long first, int n, int4* triplets, double* w, cudaStream_t stream);
+//   S[t] = sum_u partial[t][u], fixed order
+cudaError_t tc_launch_reduce_units(const double* partial, int n_trip, int n_units, double* S, cudaStream_t stream);
+//   *E = sum_t w[t] * S[t], fixed order, one block
+cudaError_t tc_launch_reduce_energy(const double* S, const double* w, long long n, double* E, cudaStream_t stream);
+
+// microbenchmarks (tc_microbench.cu)
+cudaError_t tc_micro_dmma(int sm_count, int iters, double* sink, cudaStream_t stream, double* flop_out);
+cudaError_t tc_micro_dfma(int sm_count, int iters, double* sink, cudaStream_t stream, double* flop_out);
+cudaError_t tc_micro_copy(void* dst, const void* src, size_t bytes, int sm_count, cudaStream_t stream);

@@ -1,0 +1,72 @@
+// tc_ctx.cu -- context lifetime, status strings, statistics.
+#include <stdlib.h>
+
+#include "tc_common.cuh"
+
+extern "C" const char* tc_status_string(tc_status s) {
+    switch (s) {
+        case TC_OK: return "TC_OK";
+        case TC_ERR_INVALID_ARG: return "TC_ERR_INVALID_ARG";
+        case TC_ERR_UNSUPPORTED_DEVICE: return "TC_ERR_UNSUPPORTED_DEVICE";
+        case TC_ERR_WORKSPACE_TOO_SMALL: return "TC_ERR_WORKSPACE_TOO_SMALL";
+        case TC_ERR_CUDA: return "TC_ERR_CUDA";
+        case TC_ERR_INTERNAL: return "TC_ERR_INTERNAL";
+    }
+    return "TC_ERR_UNKNOWN";
+}
+
+extern "C" const char* tc_last_error(const tc_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+extern "C" tc_status tc_create(tc_ctx** out, int device) {
+    if (!out) return TC_ERR_INVALID_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return TC_ERR_UNSUPPORTED_DEVICE;  // no CUDA device: there is no fallback path by design
+    }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return TC_ERR_CUDA;
+    if (prop.major != 10) return TC_ERR_UNSUPPORTED_DEVICE;  // kernels are built for sm_100a only
+    tc_ctx* ctx = (tc_ctx*)calloc(1, sizeof(tc_ctx));
+    if (!ctx) return TC_ERR_INTERNAL;
+    ctx->device = device;
+    ctx->sm_count = prop.multiProcessorCount;
+    ctx->cc_major = prop.major;
+    ctx->cc_minor = prop.minor;
+    ctx->smem_optin = prop.sharedMemPerBlockOptin;
+    ctx->l2_bytes = (size_t)prop.l2CacheSize;
+    ctx->err[0] = 0;
+    bool ok = cudaSetDevice(device) == cudaSuccess;
+    ok = ok && cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) == cudaSuccess;
+    cudaEvent_t* timed[6] = {&ctx->ev_t0, &ctx->ev_t1, &ctx->ev_s0, &ctx->ev_s1, &ctx->ev_c0, &ctx->ev_c1};
+    for (int n = 0; n < 6; n++) ok = ok && cudaEventCreate(timed[n]) == cudaSuccess;
+    ok = ok && cudaMallocHost(&ctx->pinned, 64 * sizeof(double)) == cudaSuccess;
+    if (!ok) {
+        tc_destroy(ctx);
+        return TC_ERR_CUDA;
+    }
+    *out = ctx;
+    return TC_OK;
+}
+
+extern "C" tc_status tc_destroy(tc_ctx* ctx) {
+    if (!ctx) return TC_ERR_INVALID_ARG;
+    cudaSetDevice(ctx->device);
+    if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
+    cudaEvent_t evs[8] = {ctx->ev_fork, ctx->ev_join, ctx->ev_t0, ctx->ev_t1,
+                          ctx->ev_s0,   ctx->ev_s1,   ctx->ev_c0, ctx->ev_c1};
+    for (int n = 0; n < 8; n++)
+        if (evs[n]) cudaEventDestroy(evs[n]);
+    if (ctx->pinned) cudaFreeHost(ctx->pinned);
+    free(ctx);
+    return TC_OK;
+}
+
+extern "C" tc_status tc_get_stats(const tc_ctx* ctx, tc_stats* out) {
+    if (!ctx || !out) return TC_ERR_INVALID_ARG;
+    *out = ctx->stats;
+    return TC_OK;
+}

@@ -1,0 +1,395 @@
+// tc_wbuild.cu -- steps a3-a6 of the hot path: the fused W-builder + epilogue.
+//
+// One CTA = one work unit = (occupied triplet i>=j>=k) x (S3-orbit of a virtual tile
+// triple {A,B,C}, A>=B>=C, tile edge T=16).  The CTA forms the up-to-six permuted
+// T^3 tiles of W_ijk (eqs. (2),(5)) in shared memory with FP64
+// tensor-core MMAs, then evaluates Y R / D (eqs. (1),(3),(4)) for every point of the
+// orbit from shared memory and writes ONE double.  W and Y never touch HBM
+// (the paper's PERMUTE kernel, Fig. 3, and the 36 global gathers of its energy
+// kernel, Fig. 4, have no counterpart here).
+//
+// Contraction algebra used:
+//   P_{xy,z}[m][n1][n2] =  sum_d t2[x][y][m][d] * vvvo[z][d][n1][n2]        particle, K = v
+//                         - sum_l ovoo[z][x][l][m] * t2[y][l][n1][n2]        hole,     K = o
+//   adds to W with the virtual index of position(x) = m, position(y) = n1, position(z) = n2,
+//   where (x,y,z) is a permutation of the occupied positions (i,j,k) -- the six rows of the
+//   table in SURVEY 8(c) step 2.  For a fixed slice z and tile pair (U,V) the families
+//   (x,y,z) and (y,x,z) share the B operand vvvo[z][:, U, V] ("slab"), so one slab step
+//   stacks them on M: a 32 x 256 x (v + 2o) DMMA GEMM whose two 16-row halves are added into
+//   two shared-memory W tiles with the index permutation folded into the store address.
+#include "tc_common.cuh"
+
+namespace {
+
+constexpr int T = 16;             // virtual tile edge
+constexpr int KC = 4;             // K chunk = one DMMA k-step
+constexpr int STAGES = 3;         // cp.async pipeline depth
+constexpr int NTHREADS = 256;
+constexpr int NWARPS = NTHREADS / 32;
+constexpr int SB = T * T + 4;     // doubles per k-row of a staged B chunk; == 4 mod 16 -> conflict-free B fragments
+constexpr int A_STAGE = 32 * KC;  // doubles
+constexpr int B_STAGE = KC * SB;  // doubles
+constexpr int TILE = T * T * T;   // doubles per W tile
+constexpr int MAX_STEPS = 18;
+
+// the six orderings of (a,b,c): even ones first.  PERM[q][p] = which of (a,b,c) sits at position p.
+__constant__ int c_perm[6][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}, {0, 2, 1}, {2, 1, 0}, {1, 0, 2}};
+
+struct StepDesc {
+    const double* Bp;     // particle B: vvvo[z] + U0*v + V0           (element + k*v*v + n1*v + n2)
+    const double* Bh[2];  // hole B of half h: t2[y or x] + U0*v + V0  (element + l*v*v + n1*v + n2)
+    const double* Ap[2];  // particle A of half h: t2[x][y] (or [y][x]) + W0*v   (element + m*v + d)
+    const double* Ah[2];  // hole A of half h: ovoo[z][x] (or [z][y]) + W0       (element + l*v + m)
+    int wW, wU, wV;       // valid extents of the m, n1, n2 tiles
+    int slot[2];          // shared-memory W tile receiving half h
+    int sm[2], sn1[2], sn2[2];  // address strides of m, n1, n2 in that tile (0 for the swizzled last coordinate)
+};
+
+struct Smem {
+    double tiles[6 * TILE];
+    double A[STAGES][A_STAGE];
+    double B[STAGES][B_STAGE];
+    StepDesc steps[MAX_STEPS];
+    double red[NWARPS];
+    int slot_of_perm[6];
+    int nsteps;
+};
+
+__device__ __forceinline__ int tile_addr(int c0, int c1, int c2) {
+    return c0 * (T * T) + c1 * T + ((c0 + c1 + c2) & (T - 1));
+}
+
+// ---- loader: one K chunk of one slab step into a pipeline stage ------------------------------
+template <int VEC>  // VEC = 2: 16-byte cp.async (v even), VEC = 1: 8-byte cp.async (any v)
+__device__ __forceinline__ void issue_chunk(Smem& s, int stage, const StepDesc& d, int phase, int k0, int o, int v) {
+    const int tid = threadIdx.x;
+    const size_t vv = (size_t)v * v;
+    const int klim = (phase == 2) ? v : o;
+    const double* Bsrc = (phase == 2) ? d.Bp : d.Bh[phase];
+    double* Bs = s.B[stage];
+    double* As = s.A[stage];
+    // B chunk: KC x T x T doubles
+    constexpr int NPIECE_B = KC * T * T / VEC;
+#pragma unroll
+    for (int p = tid; p < NPIECE_B; p += NTHREADS) {
+        const int n2 = (p % (T / VEC)) * VEC;
+        const int n1 = (p / (T / VEC)) % T;
+        const int kk = p / (T * T / VEC);
+        const bool row_ok = (k0 + kk < klim) && (n1 < d.wU);
+        int nvalid = d.wV - n2;
+        nvalid = row_ok ? (nvalid < 0 ? 0 : (nvalid > VEC ? VEC : nvalid)) : 0;
+        const double* src = nvalid ? Bsrc + (size_t)(k0 + kk) * vv + (size_t)n1 * v + n2 : Bsrc;
+        const uint32_t dst = smem_u32(Bs + kk * SB + n1 * T + n2);
+        if (VEC == 2) cp_async16(dst, src, nvalid * 8);
+        else cp_async8(dst, src, nvalid * 8);
+    }
+    // A chunk
+    if (phase == 2) {
+        constexpr int NPIECE_A = 32 * KC / VEC;
+        if (tid < NPIECE_A) {
+            const int row = tid / (KC / VEC);
+            const int kk = (tid % (KC / VEC)) * VEC;
+            const int h = row >> 4, m = row & 15;
+            int nvalid = v - (k0 + kk);
+            nvalid = (m < d.wW) ? (nvalid < 0 ? 0 : (nvalid > VEC ? VEC : nvalid)) : 0;
+            const double* src = nvalid ? d.Ap[h] + (size_t)m * v + k0 + kk : d.Ap[h];
+            const uint32_t dst = smem_u32(As + row * KC + kk);
+            if (VEC == 2) cp_async16(dst, src, nvalid * 8);
+            else cp_async8(dst, src, nvalid * 8);
+        }
+    } else {
+        if (tid < 16 * KC) {
+            const int m = tid & 15, kk = tid >> 4;
+            const bool ok = (k0 + kk < o) && (m < d.wW);
+            const double* src = ok ? d.Ah[phase] + (size_t)(k0 + kk) * v + m : d.Ah[phase];
+            cp_async8(smem_u32(As + (phase * 16 + m) * KC + kk), src, ok ? 8 : 0);
+        }
+    }
+}
+
+// ---- the kernel ----------------------------------------------------------------------------
+template <int VEC>
+__global__ void __launch_bounds__(NTHREADS, 1) k_wbuild(const tc_wbuild_args a, const int4* __restrict__ orbits) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Smem& s = *reinterpret_cast<Smem*>(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int o = a.o, v = a.v;
+
+    const int trip = blockIdx.x / a.n_orbits;
+    const int orbit = blockIdx.x - trip * a.n_orbits;
+    const int4 tr = a.triplets[trip];
+    const int occ[3] = {tr.x, tr.y, tr.z};
+    const int4 ob = orbits[orbit];
+    const int bv[3] = {ob.x, ob.y, ob.z};  // tile indices A >= B >= C
+    if (occ[0] == occ[1] && occ[1] == occ[2] && !a.W_debug) {
+        // weight 2 - d_ij - d_jk = 0 (and S_iii = 0 anyway: R vanishes by symmetry)
+        if (tid == 0) a.partial[(size_t)tr.w * a.n_orbits + orbit] = 0.0;
+        return;
+    }
+
+    // ---- zero the W tiles; thread 0 builds the step program ----
+    for (int n = tid; n < 6 * TILE; n += NTHREADS) s.tiles[n] = 0.0;
+    if (tid == 0) {
+        int sop[6];
+        for (int q = 0; q < 6; q++) {
+            sop[q] = q;
+            for (int q2 = 0; q2 < q; q2++) {
+                if (bv[c_perm[q2][0]] == bv[c_perm[q][0]] && bv[c_perm[q2][1]] == bv[c_perm[q][1]] &&
+                    bv[c_perm[q2][2]] == bv[c_perm[q][2]]) {
+                    sop[q] = q2;
+                    break;
+                }
+            }
+            s.slot_of_perm[q] = sop[q];
+        }
+        int ns = 0;
+        const size_t vv = (size_t)v * v;
+        for (int q = 0; q < 6; q++) {
+            if (sop[q] != q) continue;  // arrangement already covered
+            const int pw = c_perm[q][0], pu = c_perm[q][1], pvv = c_perm[q][2];  // which of (A,B,C) is the m / n1 / n2 tile
+            const int W0 = bv[pw] * T, U0 = bv[pu] * T, V0 = bv[pvv] * T;
+            for (int zp = 0; zp < 3; zp++) {
+                const int xp = (zp == 0) ? 1 : 0;
+                const int yp = (zp == 2) ? 1 : 2;
+                const int ox = occ[xp], oy = occ[yp], oz = occ[zp];
+                StepDesc& d = s.steps[ns++];
+                d.Bp = a.slice_ptr[oz] + (size_t)U0 * v + V0;
+                d.Bh[0] = a.t2 + (size_t)oy * o * vv + (size_t)U0 * v + V0;
+                d.Bh[1] = a.t2 + (size_t)ox * o * vv + (size_t)U0 * v + V0;
+                d.Ap[0] = a.t2 + ((size_t)ox * o + oy) * vv + (size_t)W0 * v;
+                d.Ap[1] = a.t2 + ((size_t)oy * o + ox) * vv + (size_t)W0 * v;
+                d.Ah[0] = a.ovoo + ((size_t)oz * o + ox) * o * v + W0;
+                d.Ah[1] = a.ovoo + ((size_t)oz * o + oy) * o * v + W0;
+                d.wW = min(T, v - W0);
+                d.wU = min(T, v - U0);
+                d.wV = min(T, v - V0);
+                for (int h = 0; h < 2; h++) {
+                    // half 0: family (x,y,z): m -> position xp, n1 -> yp, n2 -> zp
+                    // half 1: family (y,x,z): m -> position yp, n1 -> xp, n2 -> zp
+                    const int pm = h ? yp : xp, pn1 = h ? xp : yp, pn2 = zp;
+                    int rho[3];  // which of (A,B,C) sits at each position of the output tile
+                    rho[pm] = pw;
+                    rho[pn1] = pu;
+                    rho[pn2] = pvv;
+                    int qq = 0;
+                    for (int q3 = 0; q3 < 6; q3++)
+                        if (c_perm[q3][0] == rho[0] && c_perm[q3][1] == rho[1] && c_perm[q3][2] == rho[2]) qq = q3;
+                    d.slot[h] = sop[qq];
+                    const int strides[3] = {T * T, T, 0};
+                    d.sm[h] = strides[pm];
+                    d.sn1[h] = strides[pn1];
+                    d.sn2[h] = strides[pn2];
+                }
+            }
+        }
+        s.nsteps = ns;
+    }
+    __syncthreads();
+
+    const int nsteps = s.nsteps;
+    const int nhc = (o + KC - 1) / KC;  // chunks per hole phase
+    const int npc = (v + KC - 1) / KC;  // chunks of the particle phase
+    const int cps = 2 * nhc + npc;      // chunks per step
+    const int total = nsteps * cps;
+
+    // accumulators: [row block 0..3][n1 index 0..1][column block 0..1][2]
+    double acc[4][2][2][2];
+#pragma unroll
+    for (int x = 0; x < 4; x++)
+#pragma unroll
+        for (int y = 0; y < 2; y++)
+#pragma unroll
+            for (int z = 0; z < 2; z++) acc[x][y][z][0] = acc[x][y][z][1] = 0.0;
+
+    // loader state (runs STAGES-1 chunks ahead of the consumer)
+    int ld_step = 0, ld_r = 0, ld_c = 0;
+    auto load_next = [&]() {
+        if (ld_c < total) {
+            const int phase = (ld_r < nhc) ? 0 : (ld_r < 2 * nhc ? 1 : 2);
+            const int k0 = (ld_r - (phase == 0 ? 0 : phase == 1 ? nhc : 2 * nhc)) * KC;
+            issue_chunk<VEC>(s, ld_c % STAGES, s.steps[ld_step], phase, k0, o, v);
+            ld_c++;
+            if (++ld_r == cps) {
+                ld_r = 0;
+                ld_step++;
+            }
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int n = 0; n < STAGES - 1; n++) load_next();
+
+    const int fr = lane >> 2, fk = lane & 3;
+    int cs_step = 0, cs_r = 0;
+    for (int c = 0; c < total; c++) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        load_next();
+
+        const int phase = (cs_r < nhc) ? 0 : (cs_r < 2 * nhc ? 1 : 2);
+        if (cs_r == 2 * nhc) {  // the hole sums enter W with a minus sign (eq. (2))
+#pragma unroll
+            for (int x = 0; x < 4; x++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int z = 0; z < 2; z++) {
+                        acc[x][y][z][0] = -acc[x][y][z][0];
+                        acc[x][y][z][1] = -acc[x][y][z][1];
+                    }
+        }
+        const double* As = s.A[c % STAGES];
+        const double* Bs = s.B[c % STAGES];
+        double bf[2][2];
+#pragma unroll
+        for (int y = 0; y < 2; y++)
+#pragma unroll
+            for (int z = 0; z < 2; z++) bf[y][z] = Bs[fk * SB + (warp + 8 * y) * T + z * 8 + fr];
+        if (phase != 1) {
+#pragma unroll
+            for (int x = 0; x < 2; x++) {
+                const double af = As[(x * 8 + fr) * KC + fk];
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int z = 0; z < 2; z++) dmma884(acc[x][y][z][0], acc[x][y][z][1], af, bf[y][z]);
+            }
+        }
+        if (phase != 0) {
+#pragma unroll
+            for (int x = 2; x < 4; x++) {
+                const double af = As[(x * 8 + fr) * KC + fk];
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int z = 0; z < 2; z++) dmma884(acc[x][y][z][0], acc[x][y][z][1], af, bf[y][z]);
+            }
+        }
+
+        if (++cs_r == cps) {
+            // ---- flush: add the two 16-row halves into their W tiles, permutation in the address ----
+            const StepDesc& d = s.steps[cs_step];
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                double* tile = s.tiles + d.slot[h] * TILE;
+                const int sm = d.sm[h], sn1 = d.sn1[h], sn2 = d.sn2[h];
+#pragma unroll
+                for (int xb = 0; xb < 2; xb++)
+#pragma unroll
+                    for (int y = 0; y < 2; y++)
+#pragma unroll
+                        for (int z = 0; z < 2; z++)
+#pragma unroll
+                            for (int e = 0; e < 2; e++) {
+                                const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
+                                const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((m + n1 + n2) & (T - 1));
+                                tile[addr] += acc[2 * h + xb][y][z][e];
+                                acc[2 * h + xb][y][z][e] = 0.0;
+                            }
+                __syncthreads();  // the two halves may hit the same tile (repeated tile index)
+            }
+            cs_r = 0;
+            cs_step++;
+        }
+    }
+    cp_async_wait<0>();
+    __syncthreads();
+
+    // ---- optional: dump W (parity tests of the contraction alone) ----
+    if (a.W_debug) {
+        for (int q = 0; q < 6; q++) {
+            if (s.slot_of_perm[q] != q) continue;
+            const int P0 = bv[c_perm[q][0]] * T, Q0 = bv[c_perm[q][1]] * T, R0 = bv[c_perm[q][2]] * T;
+            for (int n = tid; n < TILE; n += NTHREADS) {
+                const int c2 = n & 15, c1 = (n >> 4) & 15, c0 = n >> 8;
+                if (P0 + c0 < v && Q0 + c1 < v && R0 + c2 < v)
+                    a.W_debug[((size_t)(P0 + c0) * v + (Q0 + c1)) * v + R0 + c2] = s.tiles[q * TILE + tile_addr(c0, c1, c2)];
+            }
+        }
+    }
+
+    // ---- fused epilogue: Y = W + Vd (eq. (3)), D (Fig. 4 l.23), sum_orbit Y R / D (eq. (1)) ----
+    const int oi = occ[0], oj = occ[1], ok = occ[2];
+    const double eocc = a.eps_occ[oi] + a.eps_occ[oj] + a.eps_occ[ok];
+    const double* t1i = a.t1 + (size_t)oi * v;
+    const double* t1j = a.t1 + (size_t)oj * v;
+    const double* t1k = a.t1 + (size_t)ok * v;
+    const size_t vv = (size_t)v * v;
+    const double* Kjk = a.ovov + ((size_t)oj * o + ok) * vv;  // (jb|kc)
+    const double* Kik = a.ovov + ((size_t)oi * o + ok) * vv;  // (ia|kc)
+    const double* Kij = a.ovov + ((size_t)oi * o + oj) * vv;  // (ia|jb)
+    const int A0 = bv[0] * T, B0 = bv[1] * T, C0 = bv[2] * T;
+    const int wA = min(T, v - A0), wB = min(T, v - B0), wC = min(T, v - C0);
+    const double* t0 = s.tiles + s.slot_of_perm[0] * TILE;
+    const double* t1p = s.tiles + s.slot_of_perm[1] * TILE;
+    const double* t2p = s.tiles + s.slot_of_perm[2] * TILE;
+    const double* t3 = s.tiles + s.slot_of_perm[3] * TILE;
+    const double* t4 = s.tiles + s.slot_of_perm[4] * TILE;
+    const double* t5 = s.tiles + s.slot_of_perm[5] * TILE;
+    double sum = 0.0;
+#define VD(p, q, r) (t1i[p] * Kjk[(size_t)(q) * v + (r)] + t1j[q] * Kik[(size_t)(p) * v + (r)] + t1k[r] * Kij[(size_t)(p) * v + (q)])
+    for (int n = tid; n < TILE; n += NTHREADS) {
+        const int lc = n & 15, lb = (n >> 4) & 15, la = n >> 8;
+        if (la < wA && lb < wB && lc < wC) {
+            const int ga = A0 + la, gb = B0 + lb, gc = C0 + lc;
+            const double w0 = t0[tile_addr(la, lb, lc)];   // W_abc
+            const double w1 = t1p[tile_addr(lb, lc, la)];  // W_bca
+            const double w2 = t2p[tile_addr(lc, la, lb)];  // W_cab
+            const double w3 = t3[tile_addr(la, lc, lb)];   // W_acb
+            const double w4 = t4[tile_addr(lc, lb, la)];   // W_cba
+            const double w5 = t5[tile_addr(lb, la, lc)];   // W_bac
+            const double y0 = w0 + VD(ga, gb, gc);
+            const double y1 = w1 + VD(gb, gc, ga);
+            const double y2 = w2 + VD(gc, ga, gb);
+            const double y3 = w3 + VD(ga, gc, gb);
+            const double y4 = w4 + VD(gc, gb, ga);
+            const double y5 = w5 + VD(gb, ga, gc);
+            const double Ce = w0 + w1 + w2, Co = w3 + w4 + w5;
+            const double Ye = y0 + y1 + y2, Yo = y3 + y4 + y5;
+            const double X = w0 * y0 + w1 * y1 + w2 * y2 + w3 * y3 + w4 * y4 + w5 * y5;
+            const double D = eocc - a.eps_vir[ga] - a.eps_vir[gb] - a.eps_vir[gc];
+            // sum over the six orderings of Y R, R = 4W_abc + W_bca + W_cab - 2W_acb - 2W_cba - 2W_bac
+            sum += (3.0 * X + (Ce - 2.0 * Co) * Ye + (Co - 2.0 * Ce) * Yo) / D;
+        }
+    }
+#undef VD
+    // every point above carried its whole 6-ordering orbit: repeated tile indices revisit orbits
+    const double wgt = (bv[0] == bv[1] && bv[1] == bv[2]) ? (1.0 / 6.0) : ((bv[0] == bv[1] || bv[1] == bv[2]) ? 0.5 : 1.0);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
+    if (lane == 0) s.red[warp] = sum;
+    __syncthreads();
+    if (tid == 0) {
+        double tot = 0.0;
+        for (int w = 0; w < NWARPS; w++) tot += s.red[w];
+        a.partial[(size_t)tr.w * a.n_orbits + orbit] = tot * wgt;
+    }
+}
+
+}  // namespace
+
+size_t tc_wbuild_smem_bytes() { return sizeof(Smem); }
+int tc_wbuild_tile() { return T; }
+int tc_wbuild_num_orbits(int v) {
+    const long long nb = (v + T - 1) / T;
+    return (int)(nb * (nb + 1) * (nb + 2) / 6);
+}
+
+cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const int4* orbits, cudaStream_t stream) {
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_wbuild<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_wbuild<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const long long nblocks = (long long)a.n_trip * a.n_orbits;
+    if (nblocks <= 0) return cudaSuccess;
+    if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    // 16-byte cp.async needs 16-byte aligned rows: v even and 16-byte aligned base pointers
+    const bool vec2 = (a.v % 2 == 0) && (((uintptr_t)a.t2 | (uintptr_t)a.ovoo) % 16 == 0) && a.slices_aligned16;
+    if (vec2) k_wbuild<2><<<(unsigned)nblocks, NTHREADS, sizeof(Smem), stream>>>(a, orbits);
+    else k_wbuild<1><<<(unsigned)nblocks, NTHREADS, sizeof(Smem), stream>>>(a, orbits);
+    return cudaGetLastError();
+}
