@@ -2,6 +2,7 @@
 // Product code: shares nothing with oracle/.
 #pragma once
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
@@ -84,6 +85,7 @@ struct tc_wbuild_args {
     const double* t2;
     const double* const* slice_ptr;  // device array [o]: slice_ptr[x] -> I_x[d][b][c] (NULL if not resident)
     bool slices_aligned16;           // every resident slice starts on a 16-byte boundary
+    const int* slice_slot;           // device array [o]: slot of slice x in the slice array the TMA map covers
     const double* ovoo;
     const double* ovov;
     const int4* triplets;            // device array [n_trip]: (i, j, k, row of partial[])
@@ -92,11 +94,23 @@ struct tc_wbuild_args {
     int n_orbits;
     double* W_debug;                 // optional v^3 output of W for n_trip == 1
 };
-size_t tc_wbuild_smem_bytes();
+// TMA descriptors of the four operand streams of the main-path kernel (tc_wbuild_tma.cu).
+struct tc_wbuild_maps {
+    CUtensorMap I;     // (vv|v.) slices   [slot][d][b][c]
+    CUtensorMap T2h;   // t2 as hole B     [y][l][n1][n2]
+    CUtensorMap T2p;   // t2 as particle A [x][y][m][d]
+    CUtensorMap Ovoo;  // (ov|oo) hole A   [z][x][l][m]
+    bool valid;        // false: v odd or a base pointer not 16-byte aligned -> cp.async fallback kernel
+};
+// slices: nslots slices of v^3 doubles, slice_stride doubles apart, starting at slice_base.
+cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, const double* slice_base, size_t slice_stride, int nslots,
+                                tc_wbuild_maps* out);
 int tc_wbuild_tile();                                  // virtual tile edge T
 int tc_wbuild_num_orbits(int v);                       // nb(nb+1)(nb+2)/6
-cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const int4* orbits /*device [n_orbits]: (A,B,C,0), A>=B>=C*/,
-                             cudaStream_t stream);
+// maps == NULL or !maps->valid: cp.async kernel (any v); else the TMA/mbarrier kernel.
+cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const tc_wbuild_maps* maps,
+                             const int4* orbits /*device [n_orbits]: (A,B,C,0), A>=B>=C*/, cudaStream_t stream);
+cudaError_t tc_launch_wbuild_cpasync(const tc_wbuild_args& a, const int4* orbits, cudaStream_t stream);
 
 // a7: deterministic reductions (tc_reduce.cu).
 //   triplets[t] = decode(first + t) as (i, j, k, t); w[t] = 2 - d_ij - d_jk

@@ -14,7 +14,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 // How the caller's workspace is carved.  Everything the compute calls need lives here
 // (pre-allocate and reuse; no device allocation inside the call).
 struct Layout {
-    size_t off_orbits, off_sliceptr, off_trip, off_w, off_S, off_partial, off_E, off_ovoo, off_ovov, off_vvvo;
+    size_t off_orbits, off_sliceptr, off_sliceslot, off_trip, off_w, off_S, off_partial, off_E, off_ovoo, off_ovov, off_vvvo;
     size_t total;
     int n_orbits;
     int batch;      // triplets per W-builder launch
@@ -39,6 +39,7 @@ bool make_layout(int o, int v, int naux, size_t budget, Layout* L) {
     };
     L->off_orbits = take(sizeof(int4) * (size_t)L->n_orbits);
     L->off_sliceptr = take(sizeof(double*) * (size_t)o);
+    L->off_sliceslot = take(sizeof(int) * (size_t)o);
     L->off_trip = take(sizeof(int4) * (size_t)L->batch);
     L->off_w = take(sizeof(double) * (size_t)ntrip);
     L->off_S = take(sizeof(double) * (size_t)ntrip);
@@ -163,6 +164,7 @@ extern "C" tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v, const do
     char* ws = (char*)workspace;
     int4* d_orbits = (int4*)(ws + L.off_orbits);
     const double** d_sliceptr = (const double**)(ws + L.off_sliceptr);
+    int* d_sliceslot = (int*)(ws + L.off_sliceslot);
     int4* d_trip = (int4*)(ws + L.off_trip);
     double* d_w = (double*)(ws + L.off_w);
     double* d_S = (double*)(ws + L.off_S);
@@ -207,7 +209,12 @@ extern "C" tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v, const do
         fill_orbits(v, orb);
         if ((int)orb.size() != L.n_orbits) TC_FAIL(ctx, TC_ERR_INTERNAL, "orbit count mismatch");
         std::vector<const double*> sp(o);
-        for (int x = 0; x < o; x++) sp[x] = vvvo + (size_t)x * slice_stride;
+        std::vector<int> slot(o);
+        for (int x = 0; x < o; x++) {
+            sp[x] = vvvo + (size_t)x * slice_stride;
+            slot[x] = x;  // all slices resident, slice x in slot x
+        }
+        TC_CUDA(ctx, cudaMemcpyAsync(d_sliceslot, slot.data(), sizeof(int) * slot.size(), cudaMemcpyHostToDevice, s));
         // pageable sources: cudaMemcpyAsync stages them before returning, so the vectors may die here
         TC_CUDA(ctx, cudaMemcpyAsync(d_orbits, orb.data(), sizeof(int4) * orb.size(), cudaMemcpyHostToDevice, s));
         TC_CUDA(ctx, cudaMemcpyAsync(d_sliceptr, sp.data(), sizeof(double*) * sp.size(), cudaMemcpyHostToDevice, s));
@@ -229,13 +236,17 @@ extern "C" tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v, const do
     a.triplets = d_trip;
     a.partial = d_partial;
     a.n_orbits = L.n_orbits;
+    a.slice_slot = d_sliceslot;
     a.W_debug = nullptr;
+    tc_wbuild_maps maps;
+    TC_CUDA(ctx, tc_wbuild_make_maps(a, vvvo, slice_stride, o, &maps));
+    if (getenv("TC_FORCE_CPASYNC")) maps.valid = false;  // testing aid: exercise the fallback kernel on even v
     TC_CUDA(ctx, cudaEventRecord(ctx->ev_c0, s));
     for (long long done = 0; done < count; done += L.batch) {
         const int nb = (int)((count - done < L.batch) ? (count - done) : L.batch);
         TC_CUDA(ctx, tc_launch_make_triplets(o, first + done, nb, d_trip, d_w + done, s));
         a.n_trip = nb;
-        TC_CUDA(ctx, tc_launch_wbuild(a, d_orbits, s));
+        TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits, s));
         TC_CUDA(ctx, tc_launch_reduce_units(d_partial, nb, L.n_orbits, d_S + done, s));
         ctx->stats.n_kernel_launches += 3;
         ctx->stats.n_work_units += (long long)nb * L.n_orbits;
@@ -332,13 +343,17 @@ extern "C" tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j,
     for (int x = 0; x < o; x++) sp[x] = blocks->vvvo + (size_t)x * v * v * v;
     // debug path: small temporaries allocated here (not a compute call of the hot path)
     char* tmp = nullptr;
-    const size_t b_orb = align_up(sizeof(int4) * orb.size()), b_sp = align_up(sizeof(double*) * o);
+    const size_t b_orb = align_up(sizeof(int4) * orb.size()), b_sp = align_up(sizeof(double*) * o + sizeof(int) * o);
     const size_t b_part = align_up(sizeof(double) * orb.size());
     const size_t b_dummy = align_up(sizeof(double) * (size_t)(o > v ? o : v) * v);
     TC_CUDA(ctx, cudaMalloc(&tmp, b_orb + b_sp + 256 + b_part + b_dummy));
     int4 trip = make_int4(i, j, k, 0);
     cudaError_t e = cudaMemcpyAsync(tmp, orb.data(), sizeof(int4) * orb.size(), cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(tmp + b_orb, sp.data(), sizeof(double*) * o, cudaMemcpyHostToDevice, s);
+    std::vector<int> slot(o);
+    for (int x = 0; x < o; x++) slot[x] = x;
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(tmp + b_orb + sizeof(double*) * o, slot.data(), sizeof(int) * o, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(tmp + b_orb + b_sp, &trip, sizeof(int4), cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemsetAsync(tmp + b_orb + b_sp + 256 + b_part, 0, b_dummy, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
@@ -359,8 +374,12 @@ extern "C" tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j,
         a.n_trip = 1;
         a.partial = (double*)(tmp + b_orb + b_sp + 256);
         a.n_orbits = (int)orb.size();
+        a.slice_slot = (const int*)(tmp + b_orb + sizeof(double*) * o);
         a.W_debug = W_dev;
-        e = tc_launch_wbuild(a, (const int4*)tmp, s);
+        tc_wbuild_maps maps;
+        e = tc_wbuild_make_maps(a, blocks->vvvo, (size_t)v * v * v, o, &maps);
+        if (getenv("TC_FORCE_CPASYNC")) maps.valid = false;
+        if (e == cudaSuccess) e = tc_launch_wbuild(a, &maps, (const int4*)tmp, s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     }
     cudaFree(tmp);

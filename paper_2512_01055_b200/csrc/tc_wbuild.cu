@@ -1,4 +1,6 @@
-// tc_wbuild.cu -- steps a3-a6 of the hot path: the fused W-builder + epilogue.
+// tc_wbuild.cu -- steps a3-a6 of the hot path: the fused W-builder + epilogue, cp.async variant.
+// This is the FALLBACK kernel for problems the TMA path cannot address (odd v: row strides that are
+// not multiples of 16 bytes).  The main path is tc_wbuild_tma.cu; both share tc_wbuild_shared.cuh.
 //
 // One CTA = one work unit = (occupied triplet i>=j>=k) x (S3-orbit of a virtual tile
 // triple {A,B,C}, A>=B>=C, tile edge T=16).  The CTA forms the up-to-six permuted
@@ -17,11 +19,14 @@
 //   (x,y,z) and (y,x,z) share the B operand vvvo[z][:, U, V] ("slab"), so one slab step
 //   stacks them on M: a 32 x 256 x (v + 2o) DMMA GEMM whose two 16-row halves are added into
 //   two shared-memory W tiles with the index permutation folded into the store address.
-#include "tc_common.cuh"
+#include "tc_wbuild_shared.cuh"
 
 namespace {
 
-constexpr int T = 16;             // virtual tile edge
+using tcw::T;
+using tcw::TILE;
+using tcw::c_perm;
+using tcw::tile_addr;
 constexpr int KC = 4;             // K chunk = one DMMA k-step
 constexpr int STAGES = 3;         // cp.async pipeline depth
 constexpr int NTHREADS = 256;
@@ -29,11 +34,7 @@ constexpr int NWARPS = NTHREADS / 32;
 constexpr int SB = T * T + 4;     // doubles per k-row of a staged B chunk; == 4 mod 16 -> conflict-free B fragments
 constexpr int A_STAGE = 32 * KC;  // doubles
 constexpr int B_STAGE = KC * SB;  // doubles
-constexpr int TILE = T * T * T;   // doubles per W tile
 constexpr int MAX_STEPS = 18;
-
-// the six orderings of (a,b,c): even ones first.  PERM[q][p] = which of (a,b,c) sits at position p.
-__constant__ int c_perm[6][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}, {0, 2, 1}, {2, 1, 0}, {1, 0, 2}};
 
 struct StepDesc {
     const double* Bp;     // particle B: vvvo[z] + U0*v + V0           (element + k*v*v + n1*v + n2)
@@ -54,10 +55,6 @@ struct Smem {
     int slot_of_perm[6];
     int nsteps;
 };
-
-__device__ __forceinline__ int tile_addr(int c0, int c1, int c2) {
-    return c0 * (T * T) + c1 * T + ((c0 + c1 + c2) & (T - 1));
-}
 
 // ---- loader: one K chunk of one slab step into a pipeline stage ------------------------------
 template <int VEC>  // VEC = 2: 16-byte cp.async (v even), VEC = 1: 8-byte cp.async (any v)
@@ -295,66 +292,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_wbuild(const tc_wbuild_args a, 
     cp_async_wait<0>();
     __syncthreads();
 
-    // ---- optional: dump W (parity tests of the contraction alone) ----
-    if (a.W_debug) {
-        for (int q = 0; q < 6; q++) {
-            if (s.slot_of_perm[q] != q) continue;
-            const int P0 = bv[c_perm[q][0]] * T, Q0 = bv[c_perm[q][1]] * T, R0 = bv[c_perm[q][2]] * T;
-            for (int n = tid; n < TILE; n += NTHREADS) {
-                const int c2 = n & 15, c1 = (n >> 4) & 15, c0 = n >> 8;
-                if (P0 + c0 < v && Q0 + c1 < v && R0 + c2 < v)
-                    a.W_debug[((size_t)(P0 + c0) * v + (Q0 + c1)) * v + R0 + c2] = s.tiles[q * TILE + tile_addr(c0, c1, c2)];
-            }
-        }
-    }
-
-    // ---- fused epilogue: Y = W + Vd (eq. (3)), D (Fig. 4 l.23), sum_orbit Y R / D (eq. (1)) ----
-    const int oi = occ[0], oj = occ[1], ok = occ[2];
-    const double eocc = a.eps_occ[oi] + a.eps_occ[oj] + a.eps_occ[ok];
-    const double* t1i = a.t1 + (size_t)oi * v;
-    const double* t1j = a.t1 + (size_t)oj * v;
-    const double* t1k = a.t1 + (size_t)ok * v;
-    const size_t vv = (size_t)v * v;
-    const double* Kjk = a.ovov + ((size_t)oj * o + ok) * vv;  // (jb|kc)
-    const double* Kik = a.ovov + ((size_t)oi * o + ok) * vv;  // (ia|kc)
-    const double* Kij = a.ovov + ((size_t)oi * o + oj) * vv;  // (ia|jb)
-    const int A0 = bv[0] * T, B0 = bv[1] * T, C0 = bv[2] * T;
-    const int wA = min(T, v - A0), wB = min(T, v - B0), wC = min(T, v - C0);
-    const double* t0 = s.tiles + s.slot_of_perm[0] * TILE;
-    const double* t1p = s.tiles + s.slot_of_perm[1] * TILE;
-    const double* t2p = s.tiles + s.slot_of_perm[2] * TILE;
-    const double* t3 = s.tiles + s.slot_of_perm[3] * TILE;
-    const double* t4 = s.tiles + s.slot_of_perm[4] * TILE;
-    const double* t5 = s.tiles + s.slot_of_perm[5] * TILE;
-    double sum = 0.0;
-#define VD(p, q, r) (t1i[p] * Kjk[(size_t)(q) * v + (r)] + t1j[q] * Kik[(size_t)(p) * v + (r)] + t1k[r] * Kij[(size_t)(p) * v + (q)])
-    for (int n = tid; n < TILE; n += NTHREADS) {
-        const int lc = n & 15, lb = (n >> 4) & 15, la = n >> 8;
-        if (la < wA && lb < wB && lc < wC) {
-            const int ga = A0 + la, gb = B0 + lb, gc = C0 + lc;
-            const double w0 = t0[tile_addr(la, lb, lc)];   // W_abc
-            const double w1 = t1p[tile_addr(lb, lc, la)];  // W_bca
-            const double w2 = t2p[tile_addr(lc, la, lb)];  // W_cab
-            const double w3 = t3[tile_addr(la, lc, lb)];   // W_acb
-            const double w4 = t4[tile_addr(lc, lb, la)];   // W_cba
-            const double w5 = t5[tile_addr(lb, la, lc)];   // W_bac
-            const double y0 = w0 + VD(ga, gb, gc);
-            const double y1 = w1 + VD(gb, gc, ga);
-            const double y2 = w2 + VD(gc, ga, gb);
-            const double y3 = w3 + VD(ga, gc, gb);
-            const double y4 = w4 + VD(gc, gb, ga);
-            const double y5 = w5 + VD(gb, ga, gc);
-            const double Ce = w0 + w1 + w2, Co = w3 + w4 + w5;
-            const double Ye = y0 + y1 + y2, Yo = y3 + y4 + y5;
-            const double X = w0 * y0 + w1 * y1 + w2 * y2 + w3 * y3 + w4 * y4 + w5 * y5;
-            const double D = eocc - a.eps_vir[ga] - a.eps_vir[gb] - a.eps_vir[gc];
-            // sum over the six orderings of Y R, R = 4W_abc + W_bca + W_cab - 2W_acb - 2W_cba - 2W_bac
-            sum += (3.0 * X + (Ce - 2.0 * Co) * Ye + (Co - 2.0 * Ce) * Yo) / D;
-        }
-    }
-#undef VD
-    // every point above carried its whole 6-ordering orbit: repeated tile indices revisit orbits
-    const double wgt = (bv[0] == bv[1] && bv[1] == bv[2]) ? (1.0 / 6.0) : ((bv[0] == bv[1] || bv[1] == bv[2]) ? 0.5 : 1.0);
+    if (a.W_debug) tcw::dump_W(s.tiles, s.slot_of_perm, bv, v, a.W_debug, tid, NTHREADS);
+    double sum = tcw::orbit_energy(s.tiles, s.slot_of_perm, bv, occ, a, tid, NTHREADS);
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
     if (lane == 0) s.red[warp] = sum;
@@ -362,20 +301,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_wbuild(const tc_wbuild_args a, 
     if (tid == 0) {
         double tot = 0.0;
         for (int w = 0; w < NWARPS; w++) tot += s.red[w];
-        a.partial[(size_t)tr.w * a.n_orbits + orbit] = tot * wgt;
+        a.partial[(size_t)tr.w * a.n_orbits + orbit] = tot;
     }
 }
 
 }  // namespace
 
-size_t tc_wbuild_smem_bytes() { return sizeof(Smem); }
-int tc_wbuild_tile() { return T; }
-int tc_wbuild_num_orbits(int v) {
-    const long long nb = (v + T - 1) / T;
-    return (int)(nb * (nb + 1) * (nb + 2) / 6);
-}
-
-cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const int4* orbits, cudaStream_t stream) {
+cudaError_t tc_launch_wbuild_cpasync(const tc_wbuild_args& a, const int4* orbits, cudaStream_t stream) {
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(k_wbuild<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));

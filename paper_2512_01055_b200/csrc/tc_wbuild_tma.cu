@@ -1,0 +1,458 @@
+// tc_wbuild_tma.cu -- steps a3-a6 of the hot path, main kernel: fused W-builder + epilogue with
+// TMA operand staging and a warp-specialised mbarrier pipeline (sm_100a).
+//
+// One CTA = one work unit = (occupied triplet i>=j>=k) x (S3-orbit of a virtual tile triple
+// {A,B,C}, A>=B>=C, tile edge T=16).  The up-to-six permuted T^3 tiles of W_ijk (eqs. (2),(5),
+// PAPER.md:42-53) live in shared memory for the whole unit (192 KB); W and Y never touch HBM.
+//
+// Contraction algebra: for a slice role z and a tile pair (U,V) the
+// families (x,y,z) and (y,x,z) share the B operand, so one step is a 32 x 256 x (v + 2o) GEMM
+//   P[m][n1][n2] =  sum_d t2[x][y][m][d] * vvvo[z][d][n1][n2]      particle, K = v   (rows 0-15: (x,y), 16-31: (y,x))
+//                 - sum_l ovoo[z][x][l][m] * t2[y][l][n1][n2]      hole,     K = o   (one 16-row half per phase)
+// whose two 16-row halves are added into two W tiles with the index permutation folded into
+// the shared-memory store address (no PERMUTE kernel).
+//
+// Roles: warp 8 (one elected lane) is the TMA producer: per K chunk of 4 it issues
+// cp.async.bulk.tensor boxes that land directly in the fragment order of mma.sync m8n8k4 f64
+//   B stage [z][n1][k][8]  <- box (8 c, 4 d, 16 b) of the slice viewed as dims (c, d, b, slot)
+//   A stage [rowblock][..] <- box (4 d, 16 m) of t2 rows (particle) or (8 m, 4 l) of (ov|oo) (hole)
+// so every fragment load of the 8 consumer warps is one conflict-free 256-byte LDS.64 and the
+// consumers execute only LDS + DMMA (+ one mbarrier wait/arrive per chunk).  Ragged tiles are
+// zero-filled by TMA; 8-blocks that are entirely outside v are neither loaded nor multiplied.
+#include "tc_wbuild_shared.cuh"
+
+namespace {
+
+using tcw::c_perm;
+using tcw::T;
+using tcw::TILE;
+
+constexpr int KC = 4;                     // K chunk = one DMMA k-step
+constexpr int STAGES = 3;                 // TMA pipeline depth (smem: 192 KB of W tiles leave 27 KB)
+constexpr int NCONS_WARPS = 8;
+constexpr int NCONS = NCONS_WARPS * 32;   // consumer threads
+constexpr int NTHREADS = NCONS + 32;      // + producer warp
+constexpr int B_STAGE = 2 * 16 * KC * 8;  // doubles: [z][n1][k][8]
+constexpr int A_STAGE = 4 * 32;           // doubles: four 8-row blocks of 32
+constexpr int MAX_STEPS = 18;
+constexpr uint32_t B_BOX_BYTES = 8 * KC * 16 * 8;  // 4096
+constexpr uint32_t AP_BOX_BYTES = KC * 16 * 8;     // 512
+constexpr uint32_t AH_BOX_BYTES = 8 * KC * 8;      // 256
+
+struct Step {
+    int U0, V0, W0;  // first virtual index of the n1, n2 and m tiles
+    int ox, oy, oz;  // occupied indices in the roles x, y, z
+    int zslot;       // slot of slice oz in the slice array
+    int nxb, ny, nz; // 8-blocks with at least one index below v: rows, n1, n2 (1 or 2)
+    int slot[2];     // shared-memory W tile receiving half h
+    int sm[2], sn1[2], sn2[2];  // address strides of m, n1, n2 in that tile (0 for the rotated last coordinate)
+};
+
+struct __align__(128) Smem {
+    double tiles[6 * TILE];
+    double B[STAGES][B_STAGE];
+    double A[STAGES][A_STAGE];
+    unsigned long long full[STAGES];
+    unsigned long long empty[STAGES];
+    Step steps[MAX_STEPS];
+    double red[NCONS_WARPS];
+    int slot_of_perm[6];
+    int nsteps;
+};
+
+// ---- mbarrier / TMA primitives -----------------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory"); }
+
+struct Frag {
+    double a[4];
+    double b[2][2];
+};
+
+// ---- the kernel ------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NTHREADS, 1)
+k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __grid_constant__ CUtensorMap mapI,
+             const __grid_constant__ CUtensorMap mapT2h, const __grid_constant__ CUtensorMap mapT2p,
+             const __grid_constant__ CUtensorMap mapOvoo) {
+    extern __shared__ unsigned char smem_raw[];
+    Smem& s = *reinterpret_cast<Smem*>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int o = a.o, v = a.v;
+
+    const int trip = blockIdx.x / a.n_orbits;
+    const int orbit = blockIdx.x - trip * a.n_orbits;
+    const int4 tr = a.triplets[trip];
+    const int occ[3] = {tr.x, tr.y, tr.z};
+    const int4 ob = orbits[orbit];
+    const int bv[3] = {ob.x, ob.y, ob.z};  // tile indices A >= B >= C
+    if (occ[0] == occ[1] && occ[1] == occ[2] && !a.W_debug) {
+        // weight 2 - d_ij - d_jk = 0 (and S_iii = 0 anyway: R vanishes by symmetry)
+        if (tid == 0) a.partial[(size_t)tr.w * a.n_orbits + orbit] = 0.0;
+        return;
+    }
+
+    // ---- the step program: thread (q, zp) writes the step of arrangement q with slice role zp ----
+    if (tid < 18) {
+        int sop[6];
+        tcw::arrangement_slots(bv, sop);
+        const int q = tid / 3, zp = tid - 3 * q;
+        int before = 0, distinct = 0;
+#pragma unroll
+        for (int q2 = 0; q2 < 6; q2++) {
+            if (sop[q2] == q2) {
+                distinct++;
+                if (q2 < q) before++;
+            }
+        }
+        if (tid == 0) {
+            s.nsteps = 3 * distinct;
+#pragma unroll
+            for (int q2 = 0; q2 < 6; q2++) s.slot_of_perm[q2] = sop[q2];
+        }
+        if (sop[q] == q) {
+            const int pw = c_perm[q][0], pu = c_perm[q][1], pvv = c_perm[q][2];  // which of (A,B,C) is the m / n1 / n2 tile
+            const int xp = (zp == 0) ? 1 : 0;
+            const int yp = (zp == 2) ? 1 : 2;
+            Step& d = s.steps[3 * before + zp];
+            d.W0 = bv[pw] * T;
+            d.U0 = bv[pu] * T;
+            d.V0 = bv[pvv] * T;
+            d.ox = occ[xp];
+            d.oy = occ[yp];
+            d.oz = occ[zp];
+            d.zslot = a.slice_slot[occ[zp]];
+            d.nxb = (v - d.W0 > 8) ? 2 : 1;
+            d.ny = (v - d.U0 > 8) ? 2 : 1;
+            d.nz = (v - d.V0 > 8) ? 2 : 1;
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                // half 0: family (x,y,z): m -> position xp, n1 -> yp, n2 -> zp
+                // half 1: family (y,x,z): m -> position yp, n1 -> xp, n2 -> zp
+                const int pm = h ? yp : xp, pn1 = h ? xp : yp, pn2 = zp;
+                int qq = 0;
+#pragma unroll
+                for (int q3 = 0; q3 < 6; q3++)
+                    if (c_perm[q3][pm] == pw && c_perm[q3][pn1] == pu && c_perm[q3][pn2] == pvv) qq = q3;
+                d.slot[h] = sop[qq];
+                d.sm[h] = (pm == 0) ? T * T : (pm == 1 ? T : 0);
+                d.sn1[h] = (pn1 == 0) ? T * T : (pn1 == 1 ? T : 0);
+                d.sn2[h] = (pn2 == 0) ? T * T : (pn2 == 1 ? T : 0);
+            }
+        }
+    }
+    if (tid == 0) {
+        for (int n = 0; n < STAGES; n++) {
+            mbar_init(smem_u32(&s.full[n]), 1);
+            mbar_init(smem_u32(&s.empty[n]), NCONS_WARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int nsteps = s.nsteps;
+    const int nhc = (o + KC - 1) / KC;  // chunks per hole phase
+    const int npc = (v + KC - 1) / KC;  // chunks of the particle phase
+    const int cps = 2 * nhc + npc;      // chunks per step
+    const int total = nsteps * cps;
+
+    if (warp == NCONS_WARPS) {
+        // =========================== producer: one elected lane issues all TMA ===========================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t wrap = 0;  // how many times the ring has wrapped
+            for (int st = 0; st < nsteps; st++) {
+                const Step d = s.steps[st];
+                for (int r = 0; r < cps; r++) {
+                    if (wrap > 0) mbar_wait(smem_u32(&s.empty[stage]), (wrap - 1) & 1);
+                    const uint32_t full = smem_u32(&s.full[stage]);
+                    const uint32_t Bd = smem_u32(&s.B[stage][0]);
+                    const uint32_t Ad = smem_u32(&s.A[stage][0]);
+                    if (r >= 2 * nhc) {
+                        const int k0 = (r - 2 * nhc) * KC;
+                        mbar_expect_tx(full, d.nz * B_BOX_BYTES + 2 * AP_BOX_BYTES);
+                        for (int z = 0; z < d.nz; z++) tma_load_4d(Bd + z * B_BOX_BYTES, &mapI, d.V0 + 8 * z, k0, d.U0, d.zslot, full);
+                        tma_load_4d(Ad, &mapT2p, k0, d.W0, d.oy, d.ox, full);                 // rows 0-15:  t2[x][y][m][d]
+                        tma_load_4d(Ad + AP_BOX_BYTES, &mapT2p, k0, d.W0, d.ox, d.oy, full);  // rows 16-31: t2[y][x][m][d]
+                    } else {
+                        const int h = (r >= nhc) ? 1 : 0;
+                        const int k0 = (r - h * nhc) * KC;
+                        const int yy = h ? d.ox : d.oy;  // B of half h: t2[y or x][l][n1][n2]
+                        const int xx = h ? d.oy : d.ox;  // A of half h: ovoo[z][x or y][l][m]
+                        mbar_expect_tx(full, d.nz * B_BOX_BYTES + d.nxb * AH_BOX_BYTES);
+                        for (int z = 0; z < d.nz; z++) tma_load_4d(Bd + z * B_BOX_BYTES, &mapT2h, d.V0 + 8 * z, k0, d.U0, yy, full);
+                        for (int xb = 0; xb < d.nxb; xb++)
+                            tma_load_4d(Ad + (2 * h + xb) * AH_BOX_BYTES, &mapOvoo, d.W0 + 8 * xb, k0, xx, d.oz, full);
+                    }
+                    if (++stage == STAGES) {
+                        stage = 0;
+                        wrap++;
+                    }
+                }
+            }
+        }
+        return;
+    }
+
+    // =========================== consumers: 8 warps, LDS + DMMA only ===========================
+    // zero the W tiles (overlaps the first TMA round trips)
+    for (int n = tid; n < 6 * TILE; n += NCONS) s.tiles[n] = 0.0;
+
+    const int fr = lane >> 2, fk = lane & 3;
+    // fragment offsets inside a stage (doubles)
+    const int offB = (warp * KC + fk) * 8 + fr;  // + z*512 + y*8*KC*8
+    const int offAp = fr * KC + fk;              // particle: block [m 8][k 4]
+    const int offAh = fk * 8 + fr;               // hole:     block [k 4][m 8]
+
+    // accumulators: [row block 0..3][n1 index 0..1][column block 0..1][2]
+    double acc[4][2][2][2];
+#pragma unroll
+    for (int x = 0; x < 4; x++)
+#pragma unroll
+        for (int y = 0; y < 2; y++)
+#pragma unroll
+            for (int z = 0; z < 2; z++) acc[x][y][z][0] = acc[x][y][z][1] = 0.0;
+
+    auto load_frags = [&](Frag& f, int stage, int ph) {
+        const double* As = s.A[stage];
+        const double* Bs = s.B[stage] + offB;
+        if (ph == 2) {
+#pragma unroll
+            for (int x = 0; x < 4; x++) f.a[x] = As[x * 32 + offAp];
+        } else if (ph == 0) {
+            f.a[0] = As[offAh];
+            f.a[1] = As[32 + offAh];
+        } else {
+            f.a[2] = As[64 + offAh];
+            f.a[3] = As[96 + offAh];
+        }
+#pragma unroll
+        for (int y = 0; y < 2; y++)
+#pragma unroll
+            for (int z = 0; z < 2; z++) f.b[y][z] = Bs[z * (16 * KC * 8) + y * (8 * KC * 8)];
+    };
+
+    Frag cur, nxt;
+    int nstage = 0;         // stage of the chunk to be fetched next
+    uint32_t nparity = 0;   // its full-barrier parity
+    auto advance = [&]() {
+        if (++nstage == STAGES) {
+            nstage = 0;
+            nparity ^= 1;
+        }
+    };
+    mbar_wait(smem_u32(&s.full[0]), 0);
+    load_frags(cur, 0, 0);
+    int cstage = 0;
+    advance();
+
+    int r = 0, st = 0;
+    int nxb = s.steps[0].nxb, ny = s.steps[0].ny, nz = s.steps[0].nz;
+    for (int c = 0; c < total; c++) {
+        const int ph = (r < nhc) ? 0 : (r < 2 * nhc ? 1 : 2);
+        const bool last = (r + 1 == cps);
+        if (c + 1 < total) {
+            const int r1 = last ? 0 : r + 1;
+            const int ph1 = (r1 < nhc) ? 0 : (r1 < 2 * nhc ? 1 : 2);
+            mbar_wait(smem_u32(&s.full[nstage]), nparity);
+            load_frags(nxt, nstage, ph1);
+        }
+        if (r == 2 * nhc) {  // the hole sums enter W with a minus sign (eq. (2))
+#pragma unroll
+            for (int x = 0; x < 4; x++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int z = 0; z < 2; z++) {
+                        acc[x][y][z][0] = -acc[x][y][z][0];
+                        acc[x][y][z][1] = -acc[x][y][z][1];
+                    }
+        }
+        // 16 (particle) or 8 (hole) DMMA.8x8x4; blocks entirely outside v are skipped (warp-uniform)
+        if (ph != 1) {
+#pragma unroll
+            for (int xb = 0; xb < 2; xb++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int z = 0; z < 2; z++)
+                        if (xb < nxb && y < ny && z < nz) dmma884(acc[xb][y][z][0], acc[xb][y][z][1], cur.a[xb], cur.b[y][z]);
+        }
+        if (ph != 0) {
+#pragma unroll
+            for (int xb = 0; xb < 2; xb++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int z = 0; z < 2; z++)
+                        if (xb < nxb && y < ny && z < nz)
+                            dmma884(acc[2 + xb][y][z][0], acc[2 + xb][y][z][1], cur.a[2 + xb], cur.b[y][z]);
+        }
+        // every DMMA that reads this chunk's fragments has been issued: hand the stage back
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&s.empty[cstage]));
+        cstage = nstage;
+        advance();
+        cur = nxt;
+
+        if (last) {
+            // ---- flush: add the two 16-row halves into their W tiles, permutation in the address ----
+            const Step& d = s.steps[st];
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                consumer_bar();  // orders this add after every earlier add to the same element (other steps / other half)
+                double* tile = s.tiles + d.slot[h] * TILE;
+                const int sm = d.sm[h], sn1 = d.sn1[h], sn2 = d.sn2[h];
+#pragma unroll
+                for (int xb = 0; xb < 2; xb++)
+#pragma unroll
+                    for (int y = 0; y < 2; y++)
+#pragma unroll
+                        for (int z = 0; z < 2; z++)
+#pragma unroll
+                            for (int e = 0; e < 2; e++) {
+                                const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
+                                const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((m + n1 + n2) & (T - 1));
+                                tile[addr] += acc[2 * h + xb][y][z][e];
+                                acc[2 * h + xb][y][z][e] = 0.0;
+                            }
+            }
+            r = 0;
+            st++;
+            if (st < nsteps) {
+                nxb = s.steps[st].nxb;
+                ny = s.steps[st].ny;
+                nz = s.steps[st].nz;
+            }
+        } else {
+            r++;
+        }
+    }
+    consumer_bar();
+
+    if (a.W_debug) tcw::dump_W(s.tiles, s.slot_of_perm, bv, v, a.W_debug, tid, NCONS);
+    double sum = tcw::orbit_energy(s.tiles, s.slot_of_perm, bv, occ, a, tid, NCONS);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
+    if (lane == 0) s.red[warp] = sum;
+    consumer_bar();
+    if (tid == 0) {
+        double tot = 0.0;
+        for (int w = 0; w < NCONS_WARPS; w++) tot += s.red[w];
+        a.partial[(size_t)tr.w * a.n_orbits + orbit] = tot;
+    }
+}
+
+// ---- host: tensor maps -----------------------------------------------------------------------
+typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                              const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+encode_fn get_encode() {
+    static encode_fn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (encode_fn)p;
+    }
+    return fn;
+}
+
+// rank-4 FP64 map; dims/strides innermost first (stride of dim 0 is implicit), strides in doubles
+bool encode4(CUtensorMap* m, const double* base, const cuuint64_t dim[4], const cuuint64_t stride_dbl[3], const cuuint32_t box[4]) {
+    encode_fn fn = get_encode();
+    if (!fn) return false;
+    cuuint64_t strides[3] = {stride_dbl[0] * 8, stride_dbl[1] * 8, stride_dbl[2] * 8};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)base, dim, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, const double* slice_base, size_t slice_stride, int nslots,
+                                tc_wbuild_maps* out) {
+    out->valid = false;
+    const cuuint64_t o = a.o, v = a.v;
+    // TMA needs 16-byte aligned bases and strides: v even, aligned pointers
+    if (v % 2 != 0 || slice_stride % 2 != 0 || nslots < 1) return cudaSuccess;
+    if ((((uintptr_t)a.t2) | ((uintptr_t)a.ovoo) | ((uintptr_t)slice_base)) % 16 != 0) return cudaSuccess;
+    bool ok = true;
+    {   // slices [slot][d][b][c] viewed as dims (c, d, b, slot)
+        const cuuint64_t dim[4] = {v, v, v, (cuuint64_t)nslots};
+        const cuuint64_t str[3] = {v * v, v, (cuuint64_t)slice_stride};
+        const cuuint32_t box[4] = {8, KC, 16, 1};
+        ok = ok && encode4(&out->I, slice_base, dim, str, box);
+    }
+    {   // t2[y][l][n1][n2] viewed as dims (n2, l, n1, y)
+        const cuuint64_t dim[4] = {v, o, v, o};
+        const cuuint64_t str[3] = {v * v, v, o * v * v};
+        const cuuint32_t box[4] = {8, KC, 16, 1};
+        ok = ok && encode4(&out->T2h, a.t2, dim, str, box);
+    }
+    {   // t2[x][y][m][d] as dims (d, m, y, x)
+        const cuuint64_t dim[4] = {v, v, o, o};
+        const cuuint64_t str[3] = {v, v * v, o * v * v};
+        const cuuint32_t box[4] = {KC, 16, 1, 1};
+        ok = ok && encode4(&out->T2p, a.t2, dim, str, box);
+    }
+    {   // ovoo[z][x][l][m] as dims (m, l, x, z)
+        const cuuint64_t dim[4] = {v, o, o, o};
+        const cuuint64_t str[3] = {v, o * v, o * o * v};
+        const cuuint32_t box[4] = {8, KC, 1, 1};
+        ok = ok && encode4(&out->Ovoo, a.ovoo, dim, str, box);
+    }
+    out->valid = ok;
+    return cudaSuccess;
+}
+
+int tc_wbuild_tile() { return T; }
+int tc_wbuild_num_orbits(int v) {
+    const long long nb = (v + T - 1) / T;
+    return (int)(nb * (nb + 1) * (nb + 2) / 6);
+}
+
+cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const tc_wbuild_maps* maps, const int4* orbits, cudaStream_t stream) {
+    if (!maps || !maps->valid) return tc_launch_wbuild_cpasync(a, orbits, stream);
+    static bool configured = false;
+    constexpr int kSmem = (int)sizeof(Smem) + 128;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_wbuild_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const long long nblocks = (long long)a.n_trip * a.n_orbits;
+    if (nblocks <= 0) return cudaSuccess;
+    if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    k_wbuild_tma<<<(unsigned)nblocks, NTHREADS, kSmem, stream>>>(a, orbits, maps->I, maps->T2h, maps->T2p, maps->Ovoo);
+    return cudaGetLastError();
+}
