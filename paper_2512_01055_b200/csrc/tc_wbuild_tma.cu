@@ -31,7 +31,7 @@ constexpr int KC = 4;                     // K chunk = one DMMA k-step
 constexpr int STAGES = 3;                 // TMA pipeline depth (smem: 192 KB of W tiles leave 27 KB)
 constexpr int NCONS_WARPS = 8;
 constexpr int NCONS = NCONS_WARPS * 32;   // consumer threads
-constexpr int NTHREADS = NCONS + 32;      // + producer warp
+constexpr int NTHREADS = NCONS + 128;     // + producer warpgroup (one elected lane issues TMA)
 constexpr int B_STAGE = 2 * 16 * KC * 8;  // doubles: [z][n1][k][8]
 constexpr int A_STAGE = 4 * 32;           // doubles: four 8-row blocks of 32
 constexpr int MAX_STEPS = 18;
@@ -92,10 +92,143 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map
 }
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory"); }
 
-struct Frag {
-    double a[4];
-    double b[2][2];
+struct ConsumerState {
+    int stage;        // ring position of the next chunk to consume
+    uint32_t parity;  // its full-barrier parity
+    int lane;
+    int nhc, npc;     // chunks per hole phase / of the particle phase
+    uint32_t full0, empty0;  // shared addresses of full[0] / empty[0]
+    uint32_t bB, bAp, bAh;   // this thread's fragment addresses in stage 0 (B, particle A, hole A)
 };
+
+__device__ __forceinline__ double lds64(uint32_t addr) {
+    double x;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(x) : "r"(addr));
+    return x;
+}
+__device__ __forceinline__ void cons_advance(ConsumerState& cs) {
+    if (++cs.stage == STAGES) {
+        cs.stage = 0;
+        cs.parity ^= 1;
+    }
+}
+// every DMMA that reads the stage's fragments has been issued: hand the stage back to the producer
+__device__ __forceinline__ void cons_release(const ConsumerState& cs, int stage) {
+    __syncwarp();
+    if (cs.lane == 0) mbar_arrive(cs.empty0 + stage * 8);
+}
+
+// One slab step of the consumer warps: hole phase of half 0, hole phase of half 1, sign flip,
+// particle phase (software-pipelined: the fragments of chunk r+1 are fetched before the DMMAs of
+// chunk r are issued).  NXB / NY / NZ = number of 8-blocks of rows / n1 / n2 that reach below v.
+template <int NXB, int NY, int NZ>
+__device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerState& cs) {
+    constexpr uint32_t BST = B_STAGE * 8, AST = A_STAGE * 8;  // stage strides in bytes
+    // ---- hole phases: rows of half h only, K = o ----
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+        for (int r = 0; r < cs.nhc; r++) {
+            mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
+            const uint32_t pa = cs.bAh + cs.stage * AST + (2 * h) * 256;
+            const uint32_t pb = cs.bB + cs.stage * BST;
+            double fa[NXB], fb[NY][NZ];
+#pragma unroll
+            for (int xb = 0; xb < NXB; xb++) fa[xb] = lds64(pa + xb * 256);
+#pragma unroll
+            for (int y = 0; y < NY; y++)
+#pragma unroll
+                for (int z = 0; z < NZ; z++) fb[y][z] = lds64(pb + z * 4096 + y * 2048);
+#pragma unroll
+            for (int xb = 0; xb < NXB; xb++)
+#pragma unroll
+                for (int y = 0; y < NY; y++)
+#pragma unroll
+                    for (int z = 0; z < NZ; z++) dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[xb], fb[y][z]);
+            cons_release(cs, cs.stage);
+            cons_advance(cs);
+        }
+    }
+    // the hole sums enter W with a minus sign (eq. (2))
+#pragma unroll
+    for (int h = 0; h < 2; h++)
+#pragma unroll
+        for (int xb = 0; xb < NXB; xb++)
+#pragma unroll
+            for (int y = 0; y < NY; y++)
+#pragma unroll
+                for (int z = 0; z < NZ; z++) {
+                    acc[2 * h + xb][y][z][0] = -acc[2 * h + xb][y][z][0];
+                    acc[2 * h + xb][y][z][1] = -acc[2 * h + xb][y][z][1];
+                }
+
+    // ---- particle phase: both halves, K = v ----
+    double fa0[2][NXB], fb0[NY][NZ], fa1[2][NXB], fb1[NY][NZ];
+    auto load = [&](double (&fa)[2][NXB], double (&fb)[NY][NZ], int stage) {
+        const uint32_t pa = cs.bAp + stage * AST;
+        const uint32_t pb = cs.bB + stage * BST;
+#pragma unroll
+        for (int h = 0; h < 2; h++)
+#pragma unroll
+            for (int xb = 0; xb < NXB; xb++) fa[h][xb] = lds64(pa + (2 * h + xb) * 256);
+#pragma unroll
+        for (int y = 0; y < NY; y++)
+#pragma unroll
+            for (int z = 0; z < NZ; z++) fb[y][z] = lds64(pb + z * 4096 + y * 2048);
+    };
+    // DMMA (h, xb, y, z) of a chunk; the first NDIAG = max(2*NXB, NY*NZ) of the rotated order below
+    // read every fragment register once, so the stage can be handed back after them.
+    constexpr int NA = 2 * NXB, NB = NY * NZ, NALL = NA * NB;
+    constexpr int NDIAG = (NA > NB) ? NA : NB;
+    constexpr int NLATE = (NALL - NDIAG >= 4) ? 4 : 0;  // DMMAs issued after the next chunk's fragment loads
+    auto mma_range = [&](const double (&fa)[2][NXB], const double (&fb)[NY][NZ], const int lo, const int hi) {
+        // enumeration n -> (ia, ib): diagonal sweeps ia = n % NA, ib = (n + n / NA) % NB when NA >= NB, else mirrored
+#pragma unroll
+        for (int n = 0; n < NALL; n++) {
+            if (n >= lo && n < hi) {
+                int ia, ib;
+                if (NA >= NB) {
+                    ia = n % NA;
+                    ib = (n % NA + n / NA) % NB;
+                } else {
+                    ib = n % NB;
+                    ia = (n % NB + n / NB) % NA;
+                }
+                const int h = ia / NXB, xb = ia % NXB, y = ib / NZ, z = ib % NZ;
+                dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[h][xb], fb[y][z]);
+            }
+        }
+    };
+    const int npc = cs.npc;
+    mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
+    load(fa0, fb0, cs.stage);
+    int st0 = cs.stage, st1 = 0;
+    cons_advance(cs);
+    int r = 0;
+    while (true) {
+        mma_range(fa0, fb0, 0, NDIAG);
+        cons_release(cs, st0);
+        mma_range(fa0, fb0, NDIAG, NALL - NLATE);
+        if (r + 1 < npc) {
+            mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
+            load(fa1, fb1, cs.stage);
+            st1 = cs.stage;
+            cons_advance(cs);
+        }
+        mma_range(fa0, fb0, NALL - NLATE, NALL);
+        if (++r == npc) break;
+        mma_range(fa1, fb1, 0, NDIAG);
+        cons_release(cs, st1);
+        mma_range(fa1, fb1, NDIAG, NALL - NLATE);
+        if (r + 1 < npc) {
+            mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
+            load(fa0, fb0, cs.stage);
+            st0 = cs.stage;
+            cons_advance(cs);
+        }
+        mma_range(fa1, fb1, NALL - NLATE, NALL);
+        if (++r == npc) break;
+    }
+}
 
 // ---- the kernel ------------------------------------------------------------------------------
 __global__ void __launch_bounds__(NTHREADS, 1)
@@ -183,9 +316,12 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     const int cps = 2 * nhc + npc;      // chunks per step
     const int total = nsteps * cps;
 
-    if (warp == NCONS_WARPS) {
+    if (warp >= NCONS_WARPS) {
         // =========================== producer: one elected lane issues all TMA ===========================
-        if (lane == 0) {
+        // registers are allocated per scheduler partition: the producer warpgroup hands its share to
+        // the consumers (168 -> 40 / 232 per thread)
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        if (warp == NCONS_WARPS && lane == 0) {
             int stage = 0;
             uint32_t wrap = 0;  // how many times the ring has wrapped
             for (int st = 0; st < nsteps; st++) {
@@ -222,14 +358,24 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     }
 
     // =========================== consumers: 8 warps, LDS + DMMA only ===========================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
     // zero the W tiles (overlaps the first TMA round trips)
     for (int n = tid; n < 6 * TILE; n += NCONS) s.tiles[n] = 0.0;
 
-    const int fr = lane >> 2, fk = lane & 3;
-    // fragment offsets inside a stage (doubles)
-    const int offB = (warp * KC + fk) * 8 + fr;  // + z*512 + y*8*KC*8
-    const int offAp = fr * KC + fk;              // particle: block [m 8][k 4]
-    const int offAh = fk * 8 + fr;               // hole:     block [k 4][m 8]
+    ConsumerState cs;
+    cs.stage = 0;
+    cs.parity = 0;
+    cs.lane = lane;
+    cs.nhc = nhc;
+    cs.npc = npc;
+    cs.full0 = smem_u32(&s.full[0]);
+    cs.empty0 = smem_u32(&s.empty[0]);
+    {
+        const int fr = lane >> 2, fk = lane & 3;
+        cs.bB = smem_u32(&s.B[0][0]) + ((warp * KC + fk) * 8 + fr) * 8;  // stage layout [z][n1][k][8]
+        cs.bAp = smem_u32(&s.A[0][0]) + (fr * KC + fk) * 8;              // particle A block [m 8][k 4]
+        cs.bAh = smem_u32(&s.A[0][0]) + (fk * 8 + fr) * 8;               // hole A block     [k 4][m 8]
+    }
 
     // accumulators: [row block 0..3][n1 index 0..1][column block 0..1][2]
     double acc[4][2][2][2];
@@ -240,119 +386,41 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
             for (int z = 0; z < 2; z++) acc[x][y][z][0] = acc[x][y][z][1] = 0.0;
 
-    auto load_frags = [&](Frag& f, int stage, int ph) {
-        const double* As = s.A[stage];
-        const double* Bs = s.B[stage] + offB;
-        if (ph == 2) {
-#pragma unroll
-            for (int x = 0; x < 4; x++) f.a[x] = As[x * 32 + offAp];
-        } else if (ph == 0) {
-            f.a[0] = As[offAh];
-            f.a[1] = As[32 + offAh];
-        } else {
-            f.a[2] = As[64 + offAh];
-            f.a[3] = As[96 + offAh];
+    for (int st = 0; st < nsteps; st++) {
+        const Step& d = s.steps[st];
+        // dispatch on the ragged-block counts: the loops inside have compile-time trip counts, so
+        // the DMMAs carry no predicates (predicated mma.sync costs a WARPSYNC + NOP each)
+        const int code = (d.nxb - 1) * 4 + (d.ny - 1) * 2 + (d.nz - 1);
+        switch (code) {
+            case 7: run_step<2, 2, 2>(acc, cs); break;
+            case 6: run_step<2, 2, 1>(acc, cs); break;
+            case 5: run_step<2, 1, 2>(acc, cs); break;
+            case 4: run_step<2, 1, 1>(acc, cs); break;
+            case 3: run_step<1, 2, 2>(acc, cs); break;
+            case 2: run_step<1, 2, 1>(acc, cs); break;
+            case 1: run_step<1, 1, 2>(acc, cs); break;
+            default: run_step<1, 1, 1>(acc, cs); break;
         }
+        // ---- flush: add the two 16-row halves into their W tiles, permutation in the address ----
+        const int fr = lane >> 2, fk = lane & 3;
 #pragma unroll
-        for (int y = 0; y < 2; y++)
-#pragma unroll
-            for (int z = 0; z < 2; z++) f.b[y][z] = Bs[z * (16 * KC * 8) + y * (8 * KC * 8)];
-    };
-
-    Frag cur, nxt;
-    int nstage = 0;         // stage of the chunk to be fetched next
-    uint32_t nparity = 0;   // its full-barrier parity
-    auto advance = [&]() {
-        if (++nstage == STAGES) {
-            nstage = 0;
-            nparity ^= 1;
-        }
-    };
-    mbar_wait(smem_u32(&s.full[0]), 0);
-    load_frags(cur, 0, 0);
-    int cstage = 0;
-    advance();
-
-    int r = 0, st = 0;
-    int nxb = s.steps[0].nxb, ny = s.steps[0].ny, nz = s.steps[0].nz;
-    for (int c = 0; c < total; c++) {
-        const int ph = (r < nhc) ? 0 : (r < 2 * nhc ? 1 : 2);
-        const bool last = (r + 1 == cps);
-        if (c + 1 < total) {
-            const int r1 = last ? 0 : r + 1;
-            const int ph1 = (r1 < nhc) ? 0 : (r1 < 2 * nhc ? 1 : 2);
-            mbar_wait(smem_u32(&s.full[nstage]), nparity);
-            load_frags(nxt, nstage, ph1);
-        }
-        if (r == 2 * nhc) {  // the hole sums enter W with a minus sign (eq. (2))
-#pragma unroll
-            for (int x = 0; x < 4; x++)
-#pragma unroll
-                for (int y = 0; y < 2; y++)
-#pragma unroll
-                    for (int z = 0; z < 2; z++) {
-                        acc[x][y][z][0] = -acc[x][y][z][0];
-                        acc[x][y][z][1] = -acc[x][y][z][1];
-                    }
-        }
-        // 16 (particle) or 8 (hole) DMMA.8x8x4; blocks entirely outside v are skipped (warp-uniform)
-        if (ph != 1) {
+        for (int h = 0; h < 2; h++) {
+            consumer_bar();  // orders this add after every earlier add to the same element (other steps / other half)
+            double* tile = s.tiles + d.slot[h] * TILE;
+            const int sm = d.sm[h], sn1 = d.sn1[h], sn2 = d.sn2[h];
 #pragma unroll
             for (int xb = 0; xb < 2; xb++)
 #pragma unroll
                 for (int y = 0; y < 2; y++)
 #pragma unroll
                     for (int z = 0; z < 2; z++)
-                        if (xb < nxb && y < ny && z < nz) dmma884(acc[xb][y][z][0], acc[xb][y][z][1], cur.a[xb], cur.b[y][z]);
-        }
-        if (ph != 0) {
 #pragma unroll
-            for (int xb = 0; xb < 2; xb++)
-#pragma unroll
-                for (int y = 0; y < 2; y++)
-#pragma unroll
-                    for (int z = 0; z < 2; z++)
-                        if (xb < nxb && y < ny && z < nz)
-                            dmma884(acc[2 + xb][y][z][0], acc[2 + xb][y][z][1], cur.a[2 + xb], cur.b[y][z]);
-        }
-        // every DMMA that reads this chunk's fragments has been issued: hand the stage back
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&s.empty[cstage]));
-        cstage = nstage;
-        advance();
-        cur = nxt;
-
-        if (last) {
-            // ---- flush: add the two 16-row halves into their W tiles, permutation in the address ----
-            const Step& d = s.steps[st];
-#pragma unroll
-            for (int h = 0; h < 2; h++) {
-                consumer_bar();  // orders this add after every earlier add to the same element (other steps / other half)
-                double* tile = s.tiles + d.slot[h] * TILE;
-                const int sm = d.sm[h], sn1 = d.sn1[h], sn2 = d.sn2[h];
-#pragma unroll
-                for (int xb = 0; xb < 2; xb++)
-#pragma unroll
-                    for (int y = 0; y < 2; y++)
-#pragma unroll
-                        for (int z = 0; z < 2; z++)
-#pragma unroll
-                            for (int e = 0; e < 2; e++) {
-                                const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
-                                const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((m + n1 + n2) & (T - 1));
-                                tile[addr] += acc[2 * h + xb][y][z][e];
-                                acc[2 * h + xb][y][z][e] = 0.0;
-                            }
-            }
-            r = 0;
-            st++;
-            if (st < nsteps) {
-                nxb = s.steps[st].nxb;
-                ny = s.steps[st].ny;
-                nz = s.steps[st].nz;
-            }
-        } else {
-            r++;
+                        for (int e = 0; e < 2; e++) {
+                            const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
+                            const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((m + n1 + n2) & (T - 1));
+                            tile[addr] += acc[2 * h + xb][y][z][e];
+                            acc[2 * h + xb][y][z][e] = 0.0;
+                        }
         }
     }
     consumer_bar();
