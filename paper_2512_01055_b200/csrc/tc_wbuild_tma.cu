@@ -90,6 +90,17 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map
         "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
         : "memory");
 }
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "elect.sync _|p, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory"); }
 
 struct ConsumerState {
@@ -175,57 +186,67 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
 #pragma unroll
             for (int z = 0; z < NZ; z++) fb[y][z] = lds64(pb + z * 4096 + y * 2048);
     };
-    // DMMA (h, xb, y, z) of a chunk; the first NDIAG = max(2*NXB, NY*NZ) of the rotated order below
-    // read every fragment register once, so the stage can be handed back after them.
-    constexpr int NA = 2 * NXB, NB = NY * NZ, NALL = NA * NB;
-    constexpr int NDIAG = (NA > NB) ? NA : NB;
-    constexpr int NLATE = (NALL - NDIAG >= 4) ? 4 : 0;  // DMMAs issued after the next chunk's fragment loads
     auto mma_range = [&](const double (&fa)[2][NXB], const double (&fb)[NY][NZ], const int lo, const int hi) {
-        // enumeration n -> (ia, ib): diagonal sweeps ia = n % NA, ib = (n + n / NA) % NB when NA >= NB, else mirrored
 #pragma unroll
-        for (int n = 0; n < NALL; n++) {
-            if (n >= lo && n < hi) {
-                int ia, ib;
-                if (NA >= NB) {
-                    ia = n % NA;
-                    ib = (n % NA + n / NA) % NB;
-                } else {
-                    ib = n % NB;
-                    ia = (n % NB + n / NB) % NA;
-                }
-                const int h = ia / NXB, xb = ia % NXB, y = ib / NZ, z = ib % NZ;
-                dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[h][xb], fb[y][z]);
-            }
-        }
+        for (int h = 0; h < 2; h++)
+#pragma unroll
+            for (int xb = 0; xb < NXB; xb++)
+#pragma unroll
+                for (int y = 0; y < NY; y++)
+#pragma unroll
+                    for (int z = 0; z < NZ; z++) {
+                        const int n = ((h * NXB + xb) * NY + y) * NZ + z;
+                        if (n >= lo && n < hi) dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[h][xb], fb[y][z]);
+                    }
     };
+    // An integer instruction that reads every fragment register: it cannot issue before the LDS
+    // results have landed, so a stage released after it is no longer being read by this warp.
+    auto touch = [&](const double (&fa)[2][NXB], const double (&fb)[NY][NZ]) {
+        uint32_t t = 0;
+#pragma unroll
+        for (int h = 0; h < 2; h++)
+#pragma unroll
+            for (int xb = 0; xb < NXB; xb++) asm volatile("{.reg .b32 lo, hi; mov.b64 {lo, hi}, %1; lop3.b32 %0, %0, lo, hi, 0x96;}" : "+r"(t) : "d"(fa[h][xb]));
+#pragma unroll
+        for (int y = 0; y < NY; y++)
+#pragma unroll
+            for (int z = 0; z < NZ; z++) asm volatile("{.reg .b32 lo, hi; mov.b64 {lo, hi}, %1; lop3.b32 %0, %0, lo, hi, 0x96;}" : "+r"(t) : "d"(fb[y][z]));
+    };
+    constexpr int NALL = 2 * NXB * NY * NZ;
+    constexpr int NLATE = (NALL >= 8) ? 4 : (NALL >= 4 ? 2 : 1);  // DMMAs issued between the next chunk's LDS and its release
     const int npc = cs.npc;
     mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
     load(fa0, fb0, cs.stage);
-    int st0 = cs.stage, st1 = 0;
+    touch(fa0, fb0);
+    cons_release(cs, cs.stage);
     cons_advance(cs);
     int r = 0;
     while (true) {
-        mma_range(fa0, fb0, 0, NDIAG);
-        cons_release(cs, st0);
-        mma_range(fa0, fb0, NDIAG, NALL - NLATE);
-        if (r + 1 < npc) {
+        mma_range(fa0, fb0, 0, NALL - NLATE);
+        const bool more0 = (r + 1 < npc);
+        if (more0) {
             mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
             load(fa1, fb1, cs.stage);
-            st1 = cs.stage;
-            cons_advance(cs);
         }
         mma_range(fa0, fb0, NALL - NLATE, NALL);
-        if (++r == npc) break;
-        mma_range(fa1, fb1, 0, NDIAG);
-        cons_release(cs, st1);
-        mma_range(fa1, fb1, NDIAG, NALL - NLATE);
-        if (r + 1 < npc) {
-            mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
-            load(fa0, fb0, cs.stage);
-            st0 = cs.stage;
+        if (more0) {
+            touch(fa1, fb1);
+            cons_release(cs, cs.stage);
             cons_advance(cs);
         }
+        if (++r == npc) break;
+        mma_range(fa1, fb1, 0, NALL - NLATE);
+        const bool more1 = (r + 1 < npc);
+        if (more1) {
+            mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
+            load(fa0, fb0, cs.stage);
+        }
         mma_range(fa1, fb1, NALL - NLATE, NALL);
+        if (more1) {
+            touch(fa0, fb0);
+            cons_release(cs, cs.stage);
+            cons_advance(cs);
+        }
         if (++r == npc) break;
     }
 }
@@ -317,42 +338,56 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     const int total = nsteps * cps;
 
     if (warp >= NCONS_WARPS) {
-        // =========================== producer: one elected lane issues all TMA ===========================
-        // registers are allocated per scheduler partition: the producer warpgroup hands its share to
-        // the consumers (168 -> 40 / 232 per thread)
+        // =========================== producers: four warps, one operand stream each ===========================
+        //   stream 0: B columns 0-7 (+ the expect_tx of the whole stage)   stream 1: B columns 8-15
+        //   stream 2: A rows of half 0 (particle) / row block 0 (hole)      stream 3: A half 1 / row block 1
+        // Splitting the issue work keeps the per-chunk instruction path of each producer short
+        // (one wait, one UTMALDG); the code is warp-uniform and one elected lane issues.
+        // Registers are allocated per scheduler partition: this warpgroup hands its share to the
+        // consumers (168 -> 40 / 232 per thread).
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-        if (warp == NCONS_WARPS && lane == 0) {
-            int stage = 0;
-            uint32_t wrap = 0;  // how many times the ring has wrapped
-            for (int st = 0; st < nsteps; st++) {
-                const Step d = s.steps[st];
-                for (int r = 0; r < cps; r++) {
-                    if (wrap > 0) mbar_wait(smem_u32(&s.empty[stage]), (wrap - 1) & 1);
-                    const uint32_t full = smem_u32(&s.full[stage]);
-                    const uint32_t Bd = smem_u32(&s.B[stage][0]);
-                    const uint32_t Ad = smem_u32(&s.A[stage][0]);
-                    if (r >= 2 * nhc) {
-                        const int k0 = (r - 2 * nhc) * KC;
-                        mbar_expect_tx(full, d.nz * B_BOX_BYTES + 2 * AP_BOX_BYTES);
-                        for (int z = 0; z < d.nz; z++) tma_load_4d(Bd + z * B_BOX_BYTES, &mapI, d.V0 + 8 * z, k0, d.U0, d.zslot, full);
-                        tma_load_4d(Ad, &mapT2p, k0, d.W0, d.oy, d.ox, full);                 // rows 0-15:  t2[x][y][m][d]
-                        tma_load_4d(Ad + AP_BOX_BYTES, &mapT2p, k0, d.W0, d.ox, d.oy, full);  // rows 16-31: t2[y][x][m][d]
-                    } else {
-                        const int h = (r >= nhc) ? 1 : 0;
-                        const int k0 = (r - h * nhc) * KC;
-                        const int yy = h ? d.ox : d.oy;  // B of half h: t2[y or x][l][n1][n2]
-                        const int xx = h ? d.oy : d.ox;  // A of half h: ovoo[z][x or y][l][m]
-                        mbar_expect_tx(full, d.nz * B_BOX_BYTES + d.nxb * AH_BOX_BYTES);
-                        for (int z = 0; z < d.nz; z++) tma_load_4d(Bd + z * B_BOX_BYTES, &mapT2h, d.V0 + 8 * z, k0, d.U0, yy, full);
-                        for (int xb = 0; xb < d.nxb; xb++)
-                            tma_load_4d(Ad + (2 * h + xb) * AH_BOX_BYTES, &mapOvoo, d.W0 + 8 * xb, k0, xx, d.oz, full);
-                    }
-                    if (++stage == STAGES) {
-                        stage = 0;
-                        wrap++;
-                    }
+        const int pw = warp - NCONS_WARPS;
+        const bool leader = elect_one();
+        const uint32_t full0 = smem_u32(&s.full[0]), empty0 = smem_u32(&s.empty[0]);
+        const uint32_t B0 = smem_u32(&s.B[0][0]), A0 = smem_u32(&s.A[0][0]);
+        int stage = 0;
+        uint32_t wrap = 0;  // how many times the ring has wrapped
+        auto stream = [&](int nchunks, const CUtensorMap* map, int kdim, int c0, int c1, int c2, int c3, uint32_t dst0,
+                          uint32_t dst_stride, bool active, uint32_t tx_bytes) {
+            for (int r = 0; r < nchunks; r++) {
+                // every stream waits, active or not: a stream that ran ahead by two ring turns would
+                // alias the barrier's phase parity
+                if (wrap > 0) mbar_wait(empty0 + stage * 8, (wrap - 1) & 1);
+                if (leader) {
+                    const uint32_t full = full0 + stage * 8;
+                    if (pw == 0) mbar_expect_tx(full, tx_bytes);
+                    if (active) tma_load_4d(dst0 + stage * dst_stride, map, kdim == 0 ? r * KC : c0, kdim == 1 ? r * KC : c1, c2, c3, full);
+                }
+                if (++stage == STAGES) {
+                    stage = 0;
+                    wrap++;
                 }
             }
+        };
+        for (int st = 0; st < nsteps; st++) {
+            const Step d = s.steps[st];
+            // hole phases: B = t2[y or x][l][n1][n2], A = ovoo[z][x or y][l][m]
+            for (int h = 0; h < 2; h++) {
+                const int yy = h ? d.ox : d.oy, xx = h ? d.oy : d.ox;
+                const uint32_t tx = d.nz * B_BOX_BYTES + d.nxb * AH_BOX_BYTES;
+                if (pw < 2)
+                    stream(nhc, &mapT2h, 1, d.V0 + 8 * pw, 0, d.U0, yy, B0 + pw * B_BOX_BYTES, B_STAGE * 8, pw < d.nz, tx);
+                else
+                    stream(nhc, &mapOvoo, 1, d.W0 + 8 * (pw - 2), 0, xx, d.oz, A0 + (2 * h + pw - 2) * AH_BOX_BYTES, A_STAGE * 8,
+                           pw - 2 < d.nxb, tx);
+            }
+            // particle phase: B = vvvo[z][d][n1][n2], A = t2[x][y][m][d] (rows 0-15) and t2[y][x][m][d] (rows 16-31)
+            const uint32_t tx = d.nz * B_BOX_BYTES + 2 * AP_BOX_BYTES;
+            if (pw < 2)
+                stream(npc, &mapI, 1, d.V0 + 8 * pw, 0, d.U0, d.zslot, B0 + pw * B_BOX_BYTES, B_STAGE * 8, pw < d.nz, tx);
+            else
+                stream(npc, &mapT2p, 0, 0, d.W0, pw == 2 ? d.oy : d.ox, pw == 2 ? d.ox : d.oy, A0 + (pw - 2) * AP_BOX_BYTES,
+                       A_STAGE * 8, true, tx);
         }
         return;
     }
