@@ -89,7 +89,7 @@ def oracle_sample(prob_cfg, seconds_target=15.0):
     """Time the CPU oracle on a bounded triplet sample of the workload; returns a cpu_baseline dict."""
     import oracle
     from paper_2512_01055_b200 import synth
-    o, v, naux, seed = synth.CONFIGS[prob_cfg]
+    o, v, naux, seed = synth.config_sizes(prob_cfg)
     p = synth.make_config(prob_cfg)
     # the sample: the last triplets of the linear index (all-distinct i>j>k, the common case)
     ntrip = oracle.triplet_count(o)
@@ -123,7 +123,7 @@ def run_reference(args):
     if rank != 0:
         return
     from paper_2512_01055_b200 import synth
-    o, v, naux, seed = synth.CONFIGS[args.config]
+    o, v, naux, seed = synth.config_sizes(args.config)
     per_step = []
     cb = None
     for s in range(args.warmup + args.steps):
@@ -157,7 +157,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     torch.cuda.set_device(local)
     ctx = binding.Context(local)
-    o, v, naux, seed = synth.CONFIGS[args.config]
+    o, v, naux, seed = synth.config_sizes(args.config)
     ntrip = binding.triplet_count(o)
     first, count = partition(ntrip, world, rank)
     if args.triplets:

@@ -153,8 +153,16 @@ def make_problem(o: int, v: int, naux: int, seed: int, sigma_B: float = 0.05,
     return prob
 
 
+def config_sizes(name: str):
+    """(o, v, naux, seed) of a named BASELINE.json config, or of an ad-hoc "o,v,naux,seed" string."""
+    if name in CONFIGS:
+        return CONFIGS[name]
+    o, v, naux, seed = (int(x) for x in name.split(","))
+    return o, v, naux, seed
+
+
 def make_config(name: str, blocks: bool = False, sigma_B: float = 0.05) -> Problem:
-    o, v, naux, seed = CONFIGS[name]
+    o, v, naux, seed = config_sizes(name)
     return make_problem(o, v, naux, seed, sigma_B=sigma_B, blocks=blocks)
 
 
