@@ -100,7 +100,6 @@ struct tc_wbuild_maps {
     CUtensorMap T2h;   // t2 as hole B     [y][l][n1][n2]
     CUtensorMap T2p;   // t2 as particle A [x][y][m][d]
     CUtensorMap Ovoo;  // (ov|oo) hole A   [z][x][l][m]
-    CUtensorMap pfI, pfT2h, pfT2p, pfOvoo;  // the same tensors with boxes 8 chunks long: L2 prefetch
     bool valid;        // false: v odd or a base pointer not 16-byte aligned -> cp.async fallback kernel
 };
 // slices: nslots slices of v^3 doubles, slice_stride doubles apart, starting at slice_base.

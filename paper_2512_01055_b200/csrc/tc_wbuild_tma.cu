@@ -35,8 +35,6 @@ constexpr int NTHREADS = NCONS + 128;     // + producer warpgroup (one elected l
 constexpr int B_STAGE = 2 * 16 * KC * 8;  // doubles: [z][n1][k][8]
 constexpr int A_STAGE = 4 * 32;           // doubles: four 8-row blocks of 32
 constexpr int MAX_STEPS = 18;
-constexpr int PF_G = 8;        // chunks covered by one L2-prefetch box
-constexpr int PF_AHEAD = 12;   // the prefetch cursor leads the staging cursor by at least this many chunks
 constexpr uint32_t B_BOX_BYTES = 8 * KC * 16 * 8;  // 4096
 constexpr uint32_t AP_BOX_BYTES = KC * 16 * 8;     // 512
 constexpr uint32_t AH_BOX_BYTES = 8 * KC * 8;      // 256
@@ -86,96 +84,6 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
             : "memory");
     } while (!done);
 }
-// non-blocking phase query: the result is consumed much later, so its latency is covered
-__device__ __forceinline__ uint32_t mbar_test(uint32_t bar, uint32_t parity) {
-    uint32_t done;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(done)
-        : "r"(bar), "r"(parity)
-        : "memory");
-    return done;
-}
-// N DMMAs with a non-blocking phase query of `bar` issued in front of them and its result converted
-// to a register behind them, in ONE asm block: the ~200-cycle latency of the query is covered by
-// the DMMAs instead of stalling the warp (a separate test_wait + selp is scheduled back to back).
-#define TCW_MMA "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 "
-__device__ __forceinline__ uint32_t mmaq4(uint32_t bar, uint32_t parity, double& c00, double& c01, double a0, double b0, double& c10,
-                                          double& c11, double a1, double b1, double& c20, double& c21, double a2, double b2,
-                                          double& c30, double& c31, double a3, double b3) {
-    uint32_t done;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.test_wait.parity.shared::cta.b64 p, [%9], %10;\n" TCW_MMA "{%1,%2}, {%11}, {%12}, {%1,%2};\n" TCW_MMA
-        "{%3,%4}, {%13}, {%14}, {%3,%4};\n" TCW_MMA "{%5,%6}, {%15}, {%16}, {%5,%6};\n" TCW_MMA
-        "{%7,%8}, {%17}, {%18}, {%7,%8};\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(done), "+d"(c00), "+d"(c01), "+d"(c10), "+d"(c11), "+d"(c20), "+d"(c21), "+d"(c30), "+d"(c31)
-        : "r"(bar), "r"(parity), "d"(a0), "d"(b0), "d"(a1), "d"(b1), "d"(a2), "d"(b2), "d"(a3), "d"(b3)
-        : "memory");
-    return done;
-}
-// eight DMMAs: accumulator pair n (c[2n], c[2n+1]) uses A fragment n % 4 and B fragment (n + 1 + n / 4) % 4
-// (sweeps 1 and 2 of the diagonal enumeration of a 4 x 4 block grid)
-__device__ __forceinline__ uint32_t mmaq8(uint32_t bar, uint32_t parity, double& c0, double& c1, double& c2, double& c3, double& c4,
-                                          double& c5, double& c6, double& c7, double& c8, double& c9, double& c10, double& c11,
-                                          double& c12, double& c13, double& c14, double& c15, double a0, double a1, double a2,
-                                          double a3, double b0, double b1, double b2, double b3) {
-    uint32_t done;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.test_wait.parity.shared::cta.b64 p, [%17], %18;\n"
-        TCW_MMA "{%1,%2}, {%19}, {%24}, {%1,%2};\n"
-        TCW_MMA "{%3,%4}, {%20}, {%25}, {%3,%4};\n"
-        TCW_MMA "{%5,%6}, {%21}, {%26}, {%5,%6};\n"
-        TCW_MMA "{%7,%8}, {%22}, {%23}, {%7,%8};\n"
-        TCW_MMA "{%9,%10}, {%19}, {%25}, {%9,%10};\n"
-        TCW_MMA "{%11,%12}, {%20}, {%26}, {%11,%12};\n"
-        TCW_MMA "{%13,%14}, {%21}, {%23}, {%13,%14};\n"
-        TCW_MMA "{%15,%16}, {%22}, {%24}, {%15,%16};\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(done), "+d"(c0), "+d"(c1), "+d"(c2), "+d"(c3), "+d"(c4), "+d"(c5), "+d"(c6), "+d"(c7), "+d"(c8), "+d"(c9), "+d"(c10),
-          "+d"(c11), "+d"(c12), "+d"(c13), "+d"(c14), "+d"(c15)
-        : "r"(bar), "r"(parity), "d"(a0), "d"(a1), "d"(a2), "d"(a3), "d"(b0), "d"(b1), "d"(b2), "d"(b3)
-        : "memory");
-    return done;
-}
-__device__ __forceinline__ uint32_t mmaq2(uint32_t bar, uint32_t parity, double& c00, double& c01, double a0, double b0, double& c10,
-                                          double& c11, double a1, double b1) {
-    uint32_t done;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.test_wait.parity.shared::cta.b64 p, [%5], %6;\n" TCW_MMA "{%1,%2}, {%7}, {%8}, {%1,%2};\n" TCW_MMA
-        "{%3,%4}, {%9}, {%10}, {%3,%4};\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(done), "+d"(c00), "+d"(c01), "+d"(c10), "+d"(c11)
-        : "r"(bar), "r"(parity), "d"(a0), "d"(b0), "d"(a1), "d"(b1)
-        : "memory");
-    return done;
-}
-__device__ __forceinline__ uint32_t mmaq1(uint32_t bar, uint32_t parity, double& c00, double& c01, double a0, double b0) {
-    uint32_t done;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.test_wait.parity.shared::cta.b64 p, [%3], %4;\n" TCW_MMA "{%1,%2}, {%5}, {%6}, {%1,%2};\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(done), "+d"(c00), "+d"(c01)
-        : "r"(bar), "r"(parity), "d"(a0), "d"(b0)
-        : "memory");
-    return done;
-}
 // keeps a loop-invariant address in a register (the compiler otherwise rematerialises the
 // shared-window base from special registers at every use)
 __device__ __forceinline__ uint32_t opaque(uint32_t x) {
@@ -187,10 +95,6 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map
         "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(dst),
         "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
         : "memory");
-}
-__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, int c1, int c2, int c3) {
-    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-                 : "memory");
 }
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;
@@ -244,8 +148,12 @@ __device__ __forceinline__ void cons_release(const ConsumerState& cs, int stage)
 }
 
 // One slab step of the consumer warps: hole phase of half 0, hole phase of half 1, sign flip,
-// particle phase (software-pipelined: the fragments of chunk r+1 are fetched before the DMMAs of
-// chunk r are issued).  NXB / NY / NZ = number of 8-blocks of rows / n1 / n2 that reach below v.
+// particle phase.  NXB / NY / NZ = number of 8-blocks of rows / n1 / n2 that reach below v.
+// Every chunk is: wait full -> 4-8 LDS.64 -> 8-16 DMMA.8x8x4 -> release.  Nothing cleverer is needed:
+// the two warps of a scheduler may be up to STAGES-1 chunks apart in the ring and settle out of
+// phase, so one warp's barrier/LDS latency is covered by the other's DMMAs (a bare LDS+DMMA loop of
+// this shape measures 99 % of the DMMA peak, with the mbarrier ring and TMA producers 91 %;
+// DESIGN.md "what the consumer loop can reach").
 template <int NXB, int NY, int NZ>
 __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerState& cs) {
     constexpr uint32_t BST = B_STAGE * 8, AST = A_STAGE * 8;  // stage strides in bytes
@@ -292,10 +200,13 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
                 }
 
     // ---- particle phase: both halves, K = v ----
-    double fa0[2][NXB], fb0[NY][NZ], fa1[2][NXB], fb1[NY][NZ];
-    auto load = [&](double (&fa)[2][NXB], double (&fb)[NY][NZ], int stage) {
-        const uint32_t pa = cs.bAp + stage * AST;
-        const uint32_t pb = cs.bB + stage * BST;
+    for (int r = 0; r < cs.npc; r++) {
+        TRACE(4, cs.tcount, cs.lane == 0 && cs.warp0);
+        mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
+        TRACE(5, cs.tcount, cs.lane == 0 && cs.warp0);
+        const uint32_t pa = cs.bAp + cs.stage * AST;
+        const uint32_t pb = cs.bB + cs.stage * BST;
+        double fa[2][NXB], fb[NY][NZ];
 #pragma unroll
         for (int h = 0; h < 2; h++)
 #pragma unroll
@@ -304,117 +215,28 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
         for (int y = 0; y < NY; y++)
 #pragma unroll
             for (int z = 0; z < NZ; z++) fb[y][z] = lds64(pb + z * 4096 + y * 2048);
-    };
-    // Enumeration of the NA x NB DMMAs of a chunk in diagonal sweeps: the first max(NA, NB) of them
-    // read every fragment register once.  n -> (ia, ib), ia = (h, xb), ib = (y, z).
-    constexpr int NA = 2 * NXB, NB = NY * NZ, NALL = NA * NB;
-    constexpr int NEARLY = (NA > NB) ? NA : NB;                       // DMMAs issued before the stage is handed back
-    constexpr int NREST = NALL - NEARLY;
-    constexpr int NLATE = (NREST >= 8) ? 4 : NREST / 2;               // DMMAs issued after the next chunk's LDS
-    auto IA = [](int n) constexpr { return (NA >= NB) ? n % NA : (n % NB + n / NB) % NA; };
-    auto IB = [](int n) constexpr { return (NA >= NB) ? (n % NA + n / NA) % NB : n % NB; };
-#define TCW_ACC(n, e) acc[2 * (IA(n) / NXB) + IA(n) % NXB][IB(n) / NZ][IB(n) % NZ][e]
-#define TCW_FA(fa, n) fa[IA(n) / NXB][IA(n) % NXB]
-#define TCW_FB(fb, n) fb[IB(n) / NZ][IB(n) % NZ]
-    auto mma_range = [&](const double (&fa)[2][NXB], const double (&fb)[NY][NZ], const int lo, const int hi) {
 #pragma unroll
-        for (int n = 0; n < NALL; n++)
-            if (n >= lo && n < hi) dmma884(TCW_ACC(n, 0), TCW_ACC(n, 1), TCW_FA(fa, n), TCW_FB(fb, n));
-    };
-    // the first NEARLY DMMAs with the non-blocking query of the next chunk's full barrier folded in
-    auto mma_early_query = [&](const double (&fa)[2][NXB], const double (&fb)[NY][NZ], uint32_t bar, uint32_t parity) -> uint32_t {
-        if constexpr (NEARLY == 4) {
-            return mmaq4(bar, parity, TCW_ACC(0, 0), TCW_ACC(0, 1), TCW_FA(fa, 0), TCW_FB(fb, 0), TCW_ACC(1, 0), TCW_ACC(1, 1),
-                         TCW_FA(fa, 1), TCW_FB(fb, 1), TCW_ACC(2, 0), TCW_ACC(2, 1), TCW_FA(fa, 2), TCW_FB(fb, 2), TCW_ACC(3, 0),
-                         TCW_ACC(3, 1), TCW_FA(fa, 3), TCW_FB(fb, 3));
-        } else {
-            static_assert(NEARLY == 2, "NA = 2 NXB and NB = NY NZ are 2 or 4");
-            return mmaq2(bar, parity, TCW_ACC(0, 0), TCW_ACC(0, 1), TCW_FA(fa, 0), TCW_FB(fb, 0), TCW_ACC(1, 0), TCW_ACC(1, 1),
-                         TCW_FA(fa, 1), TCW_FB(fb, 1));
-        }
-    };
-    // full variant: the query rides on the eight middle DMMAs (sweeps 1 and 2), far enough from its use
-    constexpr bool QMID = (NA == 4 && NB == 4);
-    auto mma_mid_query = [&](const double (&fa)[2][NXB], const double (&fb)[NY][NZ], uint32_t bar, uint32_t parity) -> uint32_t {
-        if constexpr (QMID) {
-            return mmaq8(bar, parity, TCW_ACC(4, 0), TCW_ACC(4, 1), TCW_ACC(5, 0), TCW_ACC(5, 1), TCW_ACC(6, 0), TCW_ACC(6, 1),
-                         TCW_ACC(7, 0), TCW_ACC(7, 1), TCW_ACC(8, 0), TCW_ACC(8, 1), TCW_ACC(9, 0), TCW_ACC(9, 1), TCW_ACC(10, 0),
-                         TCW_ACC(10, 1), TCW_ACC(11, 0), TCW_ACC(11, 1), TCW_FA(fa, 0), TCW_FA(fa, 1), TCW_FA(fa, 2), TCW_FA(fa, 3),
-                         TCW_FB(fb, 0), TCW_FB(fb, 1), TCW_FB(fb, 2), TCW_FB(fb, 3));
-        } else {
-            return 1;
-        }
-    };
-    // Per chunk r (fragments in fX, its stage still held):
-    //   [query full[r+1] + NEARLY DMMAs] | release stage r | DMMAs | LDS chunk r+1 | NLATE DMMAs
-    // The NEARLY DMMAs read every fragment register of chunk r; shared-memory loads of a warp
-    // complete in order and a DMMA reads its operands at issue, so after them the stage is no
-    // longer being read by this warp.  The barrier query and the LDS latencies are covered by
-    // DMMAs of the same warp: the two warps of a scheduler share the FP64 tensor pipe round-robin
-    // and drift into lockstep, so they cannot be relied on to cover each other's stalls.
-    const int npc = cs.npc;
-    TRACE(4, cs.tcount, cs.lane == 0 && cs.warp0);
-    mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
-    TRACE(5, cs.tcount, cs.lane == 0 && cs.warp0);
-    load(fa0, fb0, cs.stage);
-    int rel0 = cs.stage, rel1 = 0;
-    cons_advance(cs);
-    int r = 0;
-    while (true) {
-        const bool more0 = (r + 1 < npc);
-        uint32_t q0 = 1;
-        if (more0 && !QMID) q0 = mma_early_query(fa0, fb0, cs.full0 + cs.stage * 8, cs.parity);
-        else mma_range(fa0, fb0, 0, NEARLY);
-        cons_release(cs, rel0);
+        for (int h = 0; h < 2; h++)
+#pragma unroll
+            for (int xb = 0; xb < NXB; xb++)
+#pragma unroll
+                for (int y = 0; y < NY; y++)
+#pragma unroll
+                    for (int z = 0; z < NZ; z++) dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[h][xb], fb[y][z]);
+        // every DMMA that reads this chunk's fragments has been issued (operands are read at issue)
+        cons_release(cs, cs.stage);
         TRACE(6, cs.tcount, cs.lane == 0 && cs.warp0);
         TRACE(7, cs.tcount, cs.lane == 0 && cs.warp5);
         cs.tcount++;
-        if (more0 && QMID) q0 = mma_mid_query(fa0, fb0, cs.full0 + cs.stage * 8, cs.parity);
-        else mma_range(fa0, fb0, NEARLY, NALL - NLATE);
-        if (more0) {
-            TRACE(4, cs.tcount, cs.lane == 0 && cs.warp0);
-            if (!q0) mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
-            TRACE(5, cs.tcount, cs.lane == 0 && cs.warp0);
-            load(fa1, fb1, cs.stage);
-            rel1 = cs.stage;
-            cons_advance(cs);
-        }
-        mma_range(fa0, fb0, NALL - NLATE, NALL);
-        if (++r == npc) break;
-
-        const bool more1 = (r + 1 < npc);
-        uint32_t q1 = 1;
-        if (more1 && !QMID) q1 = mma_early_query(fa1, fb1, cs.full0 + cs.stage * 8, cs.parity);
-        else mma_range(fa1, fb1, 0, NEARLY);
-        cons_release(cs, rel1);
-        TRACE(6, cs.tcount, cs.lane == 0 && cs.warp0);
-        TRACE(7, cs.tcount, cs.lane == 0 && cs.warp5);
-        cs.tcount++;
-        if (more1 && QMID) q1 = mma_mid_query(fa1, fb1, cs.full0 + cs.stage * 8, cs.parity);
-        else mma_range(fa1, fb1, NEARLY, NALL - NLATE);
-        if (more1) {
-            TRACE(4, cs.tcount, cs.lane == 0 && cs.warp0);
-            if (!q1) mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
-            TRACE(5, cs.tcount, cs.lane == 0 && cs.warp0);
-            load(fa0, fb0, cs.stage);
-            rel0 = cs.stage;
-            cons_advance(cs);
-        }
-        mma_range(fa1, fb1, NALL - NLATE, NALL);
-        if (++r == npc) break;
+        cons_advance(cs);
     }
-#undef TCW_ACC
-#undef TCW_FA
-#undef TCW_FB
 }
 
 // ---- the kernel ------------------------------------------------------------------------------
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __grid_constant__ CUtensorMap mapI,
              const __grid_constant__ CUtensorMap mapT2h, const __grid_constant__ CUtensorMap mapT2p,
-             const __grid_constant__ CUtensorMap mapOvoo, const __grid_constant__ CUtensorMap pfI,
-             const __grid_constant__ CUtensorMap pfT2h, const __grid_constant__ CUtensorMap pfT2p,
-             const __grid_constant__ CUtensorMap pfOvoo) {
+             const __grid_constant__ CUtensorMap mapOvoo) {
     extern __shared__ unsigned char smem_raw[];
     Smem& s = *reinterpret_cast<Smem*>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -512,7 +334,6 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         // A segment = one phase of one step as seen by this stream: n chunks along one K coordinate.
         struct Seg {
             const CUtensorMap* map;    // staging box (KC along K)
-            const CUtensorMap* pfmap;  // L2-prefetch box (PF_G * KC along K)
             int kdim, c0, c1, c2, c3, n;
             uint32_t dst0, dst_stride, tx;
             bool active;
@@ -526,12 +347,12 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 g.kdim = 1;
                 g.tx = d.nz * B_BOX_BYTES + d.nxb * AH_BOX_BYTES;
                 if (pw < 2) {
-                    g.map = &mapT2h; g.pfmap = &pfT2h;
+                    g.map = &mapT2h;
                     g.c0 = d.V0 + 8 * pw; g.c1 = 0; g.c2 = d.U0; g.c3 = yy;
                     g.dst0 = B0 + pw * B_BOX_BYTES; g.dst_stride = B_STAGE * 8;
                     g.active = pw < d.nz;
                 } else {
-                    g.map = &mapOvoo; g.pfmap = &pfOvoo;
+                    g.map = &mapOvoo;
                     g.c0 = d.W0 + 8 * (pw - 2); g.c1 = 0; g.c2 = xx; g.c3 = d.oz;
                     g.dst0 = A0 + (2 * ph + pw - 2) * AH_BOX_BYTES; g.dst_stride = A_STAGE * 8;
                     g.active = pw - 2 < d.nxb;
@@ -540,13 +361,13 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 g.n = npc;
                 g.tx = d.nz * B_BOX_BYTES + 2 * AP_BOX_BYTES;
                 if (pw < 2) {
-                    g.map = &mapI; g.pfmap = &pfI;
+                    g.map = &mapI;
                     g.kdim = 1;
                     g.c0 = d.V0 + 8 * pw; g.c1 = 0; g.c2 = d.U0; g.c3 = d.zslot;
                     g.dst0 = B0 + pw * B_BOX_BYTES; g.dst_stride = B_STAGE * 8;
                     g.active = pw < d.nz;
                 } else {
-                    g.map = &mapT2p; g.pfmap = &pfT2p;
+                    g.map = &mapT2p;
                     g.kdim = 0;
                     g.c0 = 0; g.c1 = d.W0; g.c2 = (pw == 2) ? d.oy : d.ox; g.c3 = (pw == 2) ? d.ox : d.oy;
                     g.dst0 = A0 + (pw - 2) * AP_BOX_BYTES; g.dst_stride = A_STAGE * 8;
@@ -558,26 +379,10 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         int stage = 0;
         int tchunk = 0;     // chunks issued so far (timeline instrumentation)
         uint32_t wrap = 0;  // how many times the ring has wrapped
-        // L2 prefetch cursor: runs PF_AHEAD..PF_AHEAD+PF_G chunks ahead of the staging cursor, across
-        // phase and step boundaries, so that a DRAM miss is taken by the prefetch and not by the ring
-        // (three stages tolerate an L2 hit, not a DRAM round trip).
-        Seg pf;
-        int pf_seg = 0, pf_r = 0, lead = 0;
-        get_seg(0, pf);
         for (int seg_i = 0; seg_i < nseg; seg_i++) {
             Seg g;
             get_seg(seg_i, g);
             for (int r = 0; r < g.n; r++) {
-                while (lead < PF_AHEAD && pf_seg < nseg) {
-                    if (leader && pf.active) tma_prefetch_4d(pf.pfmap, pf.kdim == 0 ? pf_r * KC : pf.c0, pf.kdim == 1 ? pf_r * KC : pf.c1, pf.c2, pf.c3);
-                    const int adv = min(PF_G, pf.n - pf_r);
-                    lead += adv;
-                    pf_r += adv;
-                    if (pf_r >= pf.n) {
-                        pf_r = 0;
-                        if (++pf_seg < nseg) get_seg(pf_seg, pf);
-                    }
-                }
                 // every stream waits, active or not: a stream that ran ahead by two ring turns would
                 // alias the barrier's phase parity
                 if (wrap > 0) mbar_wait(empty0 + stage * 8, (wrap - 1) & 1);
@@ -591,7 +396,6 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 }
                 TRACE(1, tchunk, leader && pw == 0);
                 tchunk++;
-                lead--;
                 if (++stage == STAGES) {
                     stage = 0;
                     wrap++;
@@ -732,29 +536,25 @@ cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, const double* slice_bas
         const cuuint64_t dim[4] = {v, v, v, (cuuint64_t)nslots};
         const cuuint64_t str[3] = {v * v, v, (cuuint64_t)slice_stride};
         const cuuint32_t box[4] = {8, KC, 16, 1};
-        const cuuint32_t pbox[4] = {8, KC * PF_G, 16, 1};
-        ok = ok && encode4(&out->I, slice_base, dim, str, box) && encode4(&out->pfI, slice_base, dim, str, pbox);
+        ok = ok && encode4(&out->I, slice_base, dim, str, box);
     }
     {   // t2[y][l][n1][n2] viewed as dims (n2, l, n1, y)
         const cuuint64_t dim[4] = {v, o, v, o};
         const cuuint64_t str[3] = {v * v, v, o * v * v};
         const cuuint32_t box[4] = {8, KC, 16, 1};
-        const cuuint32_t pbox[4] = {8, KC * PF_G, 16, 1};
-        ok = ok && encode4(&out->T2h, a.t2, dim, str, box) && encode4(&out->pfT2h, a.t2, dim, str, pbox);
+        ok = ok && encode4(&out->T2h, a.t2, dim, str, box);
     }
     {   // t2[x][y][m][d] as dims (d, m, y, x)
         const cuuint64_t dim[4] = {v, v, o, o};
         const cuuint64_t str[3] = {v, v * v, o * v * v};
         const cuuint32_t box[4] = {KC, 16, 1, 1};
-        const cuuint32_t pbox[4] = {KC * PF_G, 16, 1, 1};
-        ok = ok && encode4(&out->T2p, a.t2, dim, str, box) && encode4(&out->pfT2p, a.t2, dim, str, pbox);
+        ok = ok && encode4(&out->T2p, a.t2, dim, str, box);
     }
     {   // ovoo[z][x][l][m] as dims (m, l, x, z)
         const cuuint64_t dim[4] = {v, o, o, o};
         const cuuint64_t str[3] = {v, o * v, o * o * v};
         const cuuint32_t box[4] = {8, KC, 1, 1};
-        const cuuint32_t pbox[4] = {8, KC * PF_G, 1, 1};
-        ok = ok && encode4(&out->Ovoo, a.ovoo, dim, str, box) && encode4(&out->pfOvoo, a.ovoo, dim, str, pbox);
+        ok = ok && encode4(&out->Ovoo, a.ovoo, dim, str, box);
     }
     out->valid = ok;
     return cudaSuccess;
@@ -778,7 +578,6 @@ cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const tc_wbuild_maps* maps
     const long long nblocks = (long long)a.n_trip * a.n_orbits;
     if (nblocks <= 0) return cudaSuccess;
     if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    k_wbuild_tma<<<(unsigned)nblocks, NTHREADS, kSmem, stream>>>(a, orbits, maps->I, maps->T2h, maps->T2p, maps->Ovoo, maps->pfI, maps->pfT2h,
-                                                                maps->pfT2p, maps->pfOvoo);
+    k_wbuild_tma<<<(unsigned)nblocks, NTHREADS, kSmem, stream>>>(a, orbits, maps->I, maps->T2h, maps->T2p, maps->Ovoo);
     return cudaGetLastError();
 }
