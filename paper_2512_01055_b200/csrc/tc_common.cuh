@@ -115,8 +115,8 @@ cudaError_t tc_launch_wbuild_cpasync(const tc_wbuild_args& a, const int4* orbits
 // a7: deterministic reductions (tc_reduce.cu).
 //   triplets[t] = decode(first + t) as (i, j, k, t); w[t] = 2 - d_ij - d_jk
 cudaError_t tc_launch_make_triplets(int o, long long first, int n, int4* triplets, double* w, cudaStream_t stream);
-//   S[t] = sum_u partial[t][u], fixed order
-cudaError_t tc_launch_reduce_units(const double* partial, int n_trip, int n_units, double* S, cudaStream_t stream);
+//   S[dest ? dest[t] : t] = sum_u partial[t][u], fixed order
+cudaError_t tc_launch_reduce_units(const double* partial, int n_trip, int n_units, const int* dest, double* S, cudaStream_t stream);
 //   *E = sum_t w[t] * S[t], fixed order, one block
 cudaError_t tc_launch_reduce_energy(const double* S, const double* w, long long n, double* E, cudaStream_t stream);
 

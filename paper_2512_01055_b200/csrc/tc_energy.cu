@@ -2,6 +2,7 @@
 // launch sequence  scheduler (a1) -> stager (a2) -> fused W-builder/epilogue (a3-a6) -> reductions (a7).
 #include <stdlib.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "tc_common.cuh"
@@ -14,7 +15,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 // How the caller's workspace is carved.  Everything the compute calls need lives here
 // (pre-allocate and reuse; no device allocation inside the call).
 struct Layout {
-    size_t off_orbits, off_sliceptr, off_sliceslot, off_trip, off_w, off_S, off_partial, off_E, off_ovoo, off_ovov, off_vvvo;
+    size_t off_orbits, off_sliceptr, off_sliceslot, off_trip, off_dest, off_w, off_S, off_partial, off_E, off_ovoo, off_ovov, off_vvvo;
     size_t total;
     int n_orbits;
     int batch;      // triplets per W-builder launch
@@ -41,6 +42,7 @@ bool make_layout(int o, int v, int naux, size_t budget, Layout* L) {
     L->off_sliceptr = take(sizeof(double*) * (size_t)o);
     L->off_sliceslot = take(sizeof(int) * (size_t)o);
     L->off_trip = take(sizeof(int4) * (size_t)L->batch);
+    L->off_dest = take(sizeof(int) * (size_t)L->batch);
     L->off_w = take(sizeof(double) * (size_t)ntrip);
     L->off_S = take(sizeof(double) * (size_t)ntrip);
     L->off_partial = take(sizeof(double) * (size_t)L->batch * L->n_orbits);
@@ -58,7 +60,8 @@ bool make_layout(int o, int v, int naux, size_t budget, Layout* L) {
             const long long fit = (long long)((budget - off) / slice_bytes);
             if (fit < slots) slots = fit;
         }
-        if (slots < o) return false;  // TODO(round 2): LRU slice cache for cfg4-size problems
+        // fewer slots than slices: the slice cache of the blocked schedule (needs i + one j + one k slice)
+        if (slots < 3 && slots < o) return false;
         L->n_slots = (int)slots;
         L->off_vvvo = take(slice_bytes * (size_t)slots);
     }
@@ -166,6 +169,7 @@ extern "C" tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v, const do
     const double** d_sliceptr = (const double**)(ws + L.off_sliceptr);
     int* d_sliceslot = (int*)(ws + L.off_sliceslot);
     int4* d_trip = (int4*)(ws + L.off_trip);
+    int* d_dest = (int*)(ws + L.off_dest);
     double* d_w = (double*)(ws + L.off_w);
     double* d_S = (double*)(ws + L.off_S);
     double* d_partial = (double*)(ws + L.off_partial);
@@ -186,7 +190,7 @@ extern "C" tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v, const do
         if (st != TC_OK) return st;
         // slices land at an aligned stride so each starts on a 256-byte boundary
         slice_stride = align_up(sizeof(double) * (size_t)v * v * v) / sizeof(double);
-        for (int x = 0; x < o; x++) {
+        for (int x = 0; x < o && L.n_slots >= o; x++) {
             TC_CUDA(ctx, tc_launch_df_gemm(df->Bvv, (size_t)v * v, df->Bov + (size_t)x * v, (size_t)o * v, v * v, v, df->naux, 1,
                                            (long long)v, 0, v, 0, 1, w_vvvo + (size_t)x * slice_stride, s));
             ctx->stats.n_kernel_launches++;
@@ -238,18 +242,123 @@ extern "C" tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v, const do
     a.n_orbits = L.n_orbits;
     a.slice_slot = d_sliceslot;
     a.W_debug = nullptr;
+    const bool blocked = df && L.n_slots < o;
+    const int nslots = blocked ? L.n_slots : o;
     tc_wbuild_maps maps;
-    TC_CUDA(ctx, tc_wbuild_make_maps(a, vvvo, slice_stride, o, &maps));
+    TC_CUDA(ctx, tc_wbuild_make_maps(a, vvvo, slice_stride, nslots, &maps));
     if (getenv("TC_FORCE_CPASYNC")) maps.valid = false;  // testing aid: exercise the fallback kernel on even v
     TC_CUDA(ctx, cudaEventRecord(ctx->ev_c0, s));
-    for (long long done = 0; done < count; done += L.batch) {
-        const int nb = (int)((count - done < L.batch) ? (count - done) : L.batch);
-        TC_CUDA(ctx, tc_launch_make_triplets(o, first + done, nb, d_trip, d_w + done, s));
-        a.n_trip = nb;
-        TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits, s));
-        TC_CUDA(ctx, tc_launch_reduce_units(d_partial, nb, L.n_orbits, d_S + done, s));
-        ctx->stats.n_kernel_launches += 3;
-        ctx->stats.n_work_units += (long long)nb * L.n_orbits;
+    if (!blocked) {
+        for (long long done = 0; done < count; done += L.batch) {
+            const int nb = (int)((count - done < L.batch) ? (count - done) : L.batch);
+            TC_CUDA(ctx, tc_launch_make_triplets(o, first + done, nb, d_trip, d_w + done, s));
+            a.n_trip = nb;
+            TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits, s));
+            TC_CUDA(ctx, tc_launch_reduce_units(d_partial, nb, L.n_orbits, nullptr, d_S + done, s));
+            ctx->stats.n_kernel_launches += 3;
+            ctx->stats.n_work_units += (long long)nb * L.n_orbits;
+        }
+    } else {
+        // ---- blocked schedule with a slice cache ("LRU of slots" for cfg4-size problems) ----
+        // The (vv|v.) slices do not all fit: nslots slots hold the slices a block of triplets needs.  For each
+        // i the (j,k) plane is cut into b x b blocks, b = (nslots-1)/2: slice i stays pinned, a block of j slices
+        // stays while the k blocks stream through, so a block of up to b^2 triplets costs at most b new slices.
+        // Missing slices are assembled from the DF factors (eq. (6)) right before the launch that needs them.
+        for (long long done = 0; done < count; done += L.batch) {  // weights of the whole range
+            const int nb = (int)((count - done < L.batch) ? (count - done) : L.batch);
+            TC_CUDA(ctx, tc_launch_make_triplets(o, first + done, nb, d_trip, d_w + done, s));
+            ctx->stats.n_kernel_launches++;
+        }
+        double* w_vvvo = (double*)(ws + L.off_vvvo);
+        const int b = std::max(1, (nslots - 1) / 2);
+        std::vector<int> slot_of(o, -1), owner(nslots, -1);
+        std::vector<long long> stamp(nslots, 0);
+        long long tick = 0;
+        std::vector<const double*> sp(o, nullptr);
+        std::vector<int4> list;
+        std::vector<int> dest;
+        auto flush_list = [&]() -> tc_status {
+            for (size_t at = 0; at < list.size(); at += (size_t)L.batch) {
+                const int nb = (int)std::min((size_t)L.batch, list.size() - at);
+                for (int t = 0; t < nb; t++) list[at + t].w = t;
+                TC_CUDA(ctx, cudaMemcpyAsync(d_trip, list.data() + at, sizeof(int4) * nb, cudaMemcpyHostToDevice, s));
+                TC_CUDA(ctx, cudaMemcpyAsync(d_dest, dest.data() + at, sizeof(int) * nb, cudaMemcpyHostToDevice, s));
+                TC_CUDA(ctx, cudaMemcpyAsync(d_sliceslot, slot_of.data(), sizeof(int) * o, cudaMemcpyHostToDevice, s));
+                TC_CUDA(ctx, cudaMemcpyAsync(d_sliceptr, sp.data(), sizeof(double*) * o, cudaMemcpyHostToDevice, s));
+                a.n_trip = nb;
+                TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits, s));
+                TC_CUDA(ctx, tc_launch_reduce_units(d_partial, nb, L.n_orbits, d_dest, d_S, s));
+                ctx->stats.n_kernel_launches += 2;
+                ctx->stats.n_work_units += (long long)nb * L.n_orbits;
+            }
+            list.clear();
+            dest.clear();
+            return TC_OK;
+        };
+        // make slice x resident without evicting any slice of `keep`
+        auto ensure = [&](int x, const std::vector<int>& keep) -> tc_status {
+            if (slot_of[x] >= 0) {
+                stamp[slot_of[x]] = ++tick;
+                return TC_OK;
+            }
+            int victim = -1;
+            for (int q = 0; q < nslots; q++) {
+                if (owner[q] >= 0 && std::find(keep.begin(), keep.end(), owner[q]) != keep.end()) continue;
+                if (victim < 0 || owner[q] < 0 || (owner[victim] >= 0 && stamp[q] < stamp[victim])) victim = q;
+                if (owner[q] < 0) break;
+            }
+            if (victim < 0) TC_FAIL(ctx, TC_ERR_INTERNAL, "slice cache: no evictable slot");
+            if (owner[victim] >= 0) {
+                slot_of[owner[victim]] = -1;
+                sp[owner[victim]] = nullptr;
+            }
+            double* dst = w_vvvo + (size_t)victim * slice_stride;
+            TC_CUDA(ctx, tc_launch_df_gemm(df->Bvv, (size_t)v * v, df->Bov + (size_t)x * v, (size_t)o * v, v * v, v, df->naux, 1,
+                                           (long long)v, 0, v, 0, 1, dst, s));
+            ctx->stats.n_kernel_launches++;
+            ctx->stats.slices_built++;
+            owner[victim] = x;
+            slot_of[x] = victim;
+            sp[x] = dst;
+            stamp[victim] = ++tick;
+            return TC_OK;
+        };
+        long long idx = first;
+        const long long end = first + count;
+        while (idx < end) {
+            int i, j, k;
+            tc_triplet_decode(o, idx, &i, &j, &k, nullptr);
+            // the (j,k) pairs of this i inside the range: idx .. min(end, start of i+1)
+            const long long next_i = (long long)(i + 1) * (i + 2) * (i + 3) / 6;
+            const long long stop = std::min(end, next_i);
+            std::vector<int4> pairs;  // (j, k, dest, 0)
+            for (long long n = idx; n < stop; n++) {
+                int ii, jj, kk;
+                tc_triplet_decode(o, n, &ii, &jj, &kk, nullptr);
+                pairs.push_back(make_int4(jj, kk, (int)(n - first), 0));
+            }
+            const int jmin = pairs.front().x, jmax = pairs.back().x;
+            for (int j0 = (jmin / b) * b; j0 <= jmax; j0 += b) {
+                for (int k0 = 0; k0 <= std::min(j0 + b - 1, jmax); k0 += b) {
+                    std::vector<int> need(1, i);
+                    for (const int4& pr : pairs) {
+                        if (pr.x < j0 || pr.x >= j0 + b || pr.y < k0 || pr.y >= k0 + b) continue;
+                        list.push_back(make_int4(i, pr.x, pr.y, 0));
+                        dest.push_back(pr.z);
+                        if (std::find(need.begin(), need.end(), pr.x) == need.end()) need.push_back(pr.x);
+                        if (std::find(need.begin(), need.end(), pr.y) == need.end()) need.push_back(pr.y);
+                    }
+                    if (list.empty()) continue;
+                    for (int x : need) {
+                        st = ensure(x, need);
+                        if (st != TC_OK) return st;
+                    }
+                    st = flush_list();
+                    if (st != TC_OK) return st;
+                }
+            }
+            idx = stop;
+        }
     }
     TC_CUDA(ctx, cudaEventRecord(ctx->ev_c1, s));
     TC_CUDA(ctx, tc_launch_reduce_energy(d_S, d_w, count, d_E, s));

@@ -39,13 +39,14 @@ __device__ __forceinline__ double block_sum_fixed(double x, double* sh) {
     return sh[0];
 }
 
-__global__ void __launch_bounds__(RT) k_reduce_units(const double* __restrict__ partial, int n_units, double* __restrict__ S) {
+__global__ void __launch_bounds__(RT) k_reduce_units(const double* __restrict__ partial, int n_units, const int* __restrict__ dest,
+                                                      double* __restrict__ S) {
     __shared__ double sh[RT];
     const double* p = partial + (size_t)blockIdx.x * n_units;
     double x = 0.0;
     for (int u = threadIdx.x; u < n_units; u += RT) x += p[u];
     x = block_sum_fixed(x, sh);
-    if (threadIdx.x == 0) S[blockIdx.x] = x;
+    if (threadIdx.x == 0) S[dest ? dest[blockIdx.x] : (int)blockIdx.x] = x;
 }
 
 __global__ void __launch_bounds__(1024) k_reduce_energy(const double* __restrict__ S, const double* __restrict__ w, long long n,
@@ -70,9 +71,9 @@ cudaError_t tc_launch_make_triplets(int o, long long first, int n, int4* triplet
     return cudaGetLastError();
 }
 
-cudaError_t tc_launch_reduce_units(const double* partial, int n_trip, int n_units, double* S, cudaStream_t stream) {
+cudaError_t tc_launch_reduce_units(const double* partial, int n_trip, int n_units, const int* dest, double* S, cudaStream_t stream) {
     if (n_trip <= 0) return cudaSuccess;
-    k_reduce_units<<<n_trip, RT, 0, stream>>>(partial, n_units, S);
+    k_reduce_units<<<n_trip, RT, 0, stream>>>(partial, n_units, dest, S);
     return cudaGetLastError();
 }
 

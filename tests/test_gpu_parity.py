@@ -137,6 +137,35 @@ def test_cfg0_scaled_twin_absolute_bound(ctx):
     assert np.abs(S - S_ref).max() <= ABS_TOL
 
 
+@pytest.mark.parametrize("nslots", [3, 4, 7])
+def test_slice_cache_blocked_schedule(ctx, nslots):
+    """DF input with a workspace too small for all (vv|v.) slices: the blocked schedule with a slice cache
+    (the cfg4 path) must give the same per-triplet S_ijk, on a full range and on a middle slice."""
+    p = synth.make_problem(9, 24, 10, 41, sigma_B=0.25, blocks=True)
+    dp = DevProblem(p)
+    o, v, naux = p.o, p.v, p.naux
+    n = oracle.triplet_count(o)
+    E_ref, S_ref = oracle.triples_energy(p)
+    full = ctx.workspace_bytes(o, v, naux)
+    slice_bytes = (v ** 3 * 8 + 255) // 256 * 256
+    budget = full - (o - nslots) * slice_bytes
+    nb = ctx.workspace_bytes(o, v, naux, budget)
+    assert nb <= budget < full
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    for first, count in ((0, n), (37, 61)):
+        S = torch.full((count,), float("nan"), dtype=torch.float64, device="cuda")
+        E = ctx.triples_energy_slice(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws, workspace_bytes=nb,
+                                     first=first, count=count, S_dev=S)
+        got = S.cpu().numpy()
+        assert np.abs(got - S_ref[first:first + count]).max() <= REL_TOL * np.abs(S_ref).max()
+        st = ctx.get_stats()
+        assert st["slices_built"] >= min(o, 3)
+    assert_energy(ctx.triples_energy_slice(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws,
+                                           workspace_bytes=nb, first=0, count=n), E_ref)
+    with pytest.raises(Exception):   # two slots cannot hold the three slices of a triplet
+        ctx.workspace_bytes(o, v, naux, full - (o - 2) * slice_bytes)
+
+
 def test_host_entry_point(ctx):
     p = synth.make_problem(4, 21, 9, 21, sigma_B=0.25, blocks=True)
     E_ref, _ = oracle.triples_energy(p)
