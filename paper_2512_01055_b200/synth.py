@@ -131,8 +131,9 @@ def mp2_amplitudes(Bov: np.ndarray, eps_occ: np.ndarray, eps_vir: np.ndarray) ->
 
 
 def make_problem(o: int, v: int, naux: int, seed: int, sigma_B: float = 0.05,
-                 sigma_t1: float = 0.01, blocks: bool = False) -> Problem:
-    """Draw one synthetic problem with the BASELINE.json recipe."""
+                 sigma_t1: float = 0.01, blocks: bool = False, with_t2: bool = True) -> Problem:
+    """Draw one synthetic problem with the BASELINE.json recipe.  with_t2=False leaves ``t2`` None (the
+    caller derives the MP2 amplitudes on the device with ``mp2_amplitudes_device``: at cfg4 size ``t2`` is 51 GB)."""
     N = o + v
     p = np.arange(N, dtype=np.uint64)
     lo = np.minimum(p[:, None], p[None, :])
@@ -146,11 +147,35 @@ def make_problem(o: int, v: int, naux: int, seed: int, sigma_B: float = 0.05,
     eps_vir = counter_uniform(seed, TENSOR_EPS_VIR, np.arange(v), 0.1, 5.0)
     t1 = counter_normal(seed, TENSOR_T1, np.arange(o * v), sigma_t1).reshape(o, v)
     Boo, Bov, Bvv = _split_B(B, o)
-    t2 = mp2_amplitudes(Bov, eps_occ, eps_vir)
+    t2 = mp2_amplitudes(Bov, eps_occ, eps_vir) if with_t2 else None
     prob = Problem(o, v, naux, eps_occ, eps_vir, np.ascontiguousarray(t1), t2, Boo, Bov, Bvv)
     if blocks:
         materialise_blocks(prob)
     return prob
+
+
+def mp2_amplitudes_device(Bov, eps_occ, eps_vir):
+    """``mp2_amplitudes`` with torch tensors on the device (input preparation for problems whose ``t2`` does not
+    fit comfortably on the host): t2[i][j][a][b] = (ia|jb) / (e_i + e_j - e_a - e_b), then made bit-exactly
+    symmetric under (i,a) <-> (j,b).  Works one occupied index at a time (temporaries of o*v*v doubles)."""
+    import torch
+    naux, o, v = Bov.shape
+    t2 = torch.empty((o, o, v, v), dtype=torch.float64, device=Bov.device)
+    Bflat = Bov.reshape(naux, o * v)
+    ea = eps_vir.reshape(v, 1, 1)
+    eb = eps_vir.reshape(1, 1, v)
+    ej = eps_occ.reshape(1, o, 1)
+    for i in range(o):
+        iajb = (Bov[:, i, :].t().contiguous() @ Bflat).reshape(v, o, v)      # [a][j][b] = (ia|jb)
+        iajb /= (eps_occ[i] + ej - ea - eb)
+        t2[i] = iajb.permute(1, 0, 2)
+        del iajb
+    for i in range(o):                                                      # t_ij^ab <- (t_ij^ab + t_ji^ba) / 2
+        avg = 0.5 * (t2[i] + t2[:, i].transpose(1, 2))
+        t2[i] = avg
+        t2[:, i] = avg.transpose(1, 2)
+        del avg
+    return t2
 
 
 def config_sizes(name: str):
@@ -161,9 +186,9 @@ def config_sizes(name: str):
     return o, v, naux, seed
 
 
-def make_config(name: str, blocks: bool = False, sigma_B: float = 0.05) -> Problem:
+def make_config(name: str, blocks: bool = False, sigma_B: float = 0.05, with_t2: bool = True) -> Problem:
     o, v, naux, seed = config_sizes(name)
-    return make_problem(o, v, naux, seed, sigma_B=sigma_B, blocks=blocks)
+    return make_problem(o, v, naux, seed, sigma_B=sigma_B, blocks=blocks, with_t2=with_t2)
 
 
 def closed_form_problem(o: int, v: int, naux: int, blocks: bool = True,

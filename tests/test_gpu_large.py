@@ -71,3 +71,40 @@ def test_cfg2_sampled(ctx):
 @pytest.mark.skipif(not os.environ.get("TC_TEST_CFG3"), reason="cfg3 (70 GB workspace, ~1 min of oracle per triplet): set TC_TEST_CFG3=1")
 def test_cfg3_sampled(ctx):
     _run_sampled(ctx, "cfg3", 2)
+
+
+@pytest.mark.skipif(not os.environ.get("TC_TEST_CFG4"), reason="cfg4 (170 GB resident, ~2.5 min of oracle per triplet): set TC_TEST_CFG4=1")
+def test_cfg4_sampled(ctx):
+    """cfg4: DF factors only, slices assembled on device into the slice cache (blocked schedule).  t2 is derived on the
+    device; the oracle gets host copies of exactly the rows and panels its loops touch for the sampled triplets
+    (the full-size host arrays are calloc'ed, so untouched pages cost nothing)."""
+    from paper_2512_01055_b200 import binding
+    name = "cfg4"
+    p = synth.make_config(name, with_t2=False)
+    o, v, naux = p.o, p.v, p.naux
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    d = {k: dev(getattr(p, k)) for k in ("eps_occ", "eps_vir", "t1", "Boo", "Bov", "Bvv")}
+    d["t2"] = synth.mp2_amplitudes_device(d["Bov"], d["eps_occ"], d["eps_vir"])
+    nb = ctx.workspace_bytes(o, v, naux, torch.cuda.mem_get_info()[0] - (3 << 30))
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    samples = [binding.triplet_index(o, 70, 31, 7), binding.triplet_index(o, 70, 31, 31)]
+    n_oracle = int(os.environ.get("TC_TEST_CFG4_TRIPLETS", "1"))
+    for idx in samples[:n_oracle]:
+        i, j, k, w = oracle.triplet_decode(o, idx)
+        S = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda")
+        ctx.triples_energy_slice(o, v, d["eps_occ"], d["eps_vir"], d["t1"], d["t2"], df=(naux, d["Boo"], d["Bov"], d["Bvv"]),
+                                 workspace=ws, workspace_bytes=nb, first=idx, count=1, S_dev=S)
+        got = float(S.cpu()[0])
+        assert ctx.get_stats()["slices_built"] == len({i, j, k})
+        occ = sorted({i, j, k})
+        p.t2 = np.zeros((o, o, v, v))
+        p.ovoo = np.zeros((o, o, o, v))
+        p.ovov = np.zeros((o, o, v, v))
+        for x in occ:
+            p.t2[x] = d["t2"][x].cpu().numpy()          # t_xl^ab for all l (hole sums) and t_xy^ad
+            for y in occ:
+                p.ovoo[x, y] = np.einsum("ql,qc->lc", p.Boo[:, :, x], p.Bov[:, y, :])     # (lx|yc)
+                p.ovov[x, y] = np.einsum("qb,qc->bc", p.Bov[:, x, :], p.Bov[:, y, :])     # (xb|yc)
+        slices = {x: synth.vvvo_slice(p, x) for x in occ}
+        _, S_ref = oracle.triples_energy_slices(p, slices, idx, 1)
+        assert abs(got - float(S_ref[0])) <= REL_TOL * abs(float(S_ref[0])), ((i, j, k), got, float(S_ref[0]))
