@@ -128,6 +128,7 @@ struct ConsumerState {
     uint32_t full0, empty0;  // shared addresses of full[0] / empty[0]
     uint32_t bB, bAp, bAh;   // this thread's fragment addresses in stage 0 (B, particle A, hole A)
     bool warp0, warp5;       // timeline instrumentation: is this consumer warp 0 / 5
+    bool skew;               // second warp of its scheduler (warps w and w+4 share one)
 };
 
 __device__ __forceinline__ double lds64(uint32_t addr) {
@@ -200,6 +201,12 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
                 }
 
     // ---- particle phase: both halves, K = v ----
+#ifdef TCW_SKEW
+    if (cs.skew) {   // experiment: start the second warp of each scheduler half a chunk late
+        const long long t0 = clock64();
+        while (clock64() - t0 < TCW_SKEW) {}
+    }
+#endif
     for (int r = 0; r < cs.npc; r++) {
         TRACE(4, cs.tcount, cs.lane == 0 && cs.warp0);
         mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
@@ -417,6 +424,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     cs.tcount = 0;
     cs.warp0 = (warp == 0);
     cs.warp5 = (warp == 5);
+    cs.skew = (warp & 4) != 0;
     cs.nhc = nhc;
     cs.npc = npc;
     cs.full0 = opaque(smem_u32(&s.full[0]));
@@ -437,6 +445,16 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
             for (int z = 0; z < 2; z++) acc[x][y][z][0] = acc[x][y][z][1] = 0.0;
 
+    // this thread's coordinates in a step's 32 x 16 x 16 result (DMMA C fragment) and their swizzle terms
+    const int fr = lane >> 2, fk = lane & 3;
+    int hm[2], hn1[2], hn2[2][2];
+#pragma unroll
+    for (int q = 0; q < 2; q++) {
+        hm[q] = tcw::swz(q * 8 + fr);
+        hn1[q] = tcw::swz(warp + 8 * q);
+        hn2[q][0] = tcw::swz(q * 8 + 2 * fk);
+        hn2[q][1] = tcw::swz(q * 8 + 2 * fk + 1);
+    }
     for (int st = 0; st < nsteps; st++) {
         const Step& d = s.steps[st];
         // dispatch on the ragged-block counts: the loops inside have compile-time trip counts, so
@@ -453,7 +471,6 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             default: run_step<1, 1, 1>(acc, cs); break;
         }
         // ---- flush: add the two 16-row halves into their W tiles, permutation in the address ----
-        const int fr = lane >> 2, fk = lane & 3;
 #pragma unroll
         for (int h = 0; h < 2; h++) {
             consumer_bar();  // orders this add after every earlier add to the same element (other steps / other half)
@@ -468,7 +485,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
                         for (int e = 0; e < 2; e++) {
                             const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
-                            const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((m + n1 + n2) & (T - 1));
+                            const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((hm[xb] + hn1[y] + hn2[z][e]) & (T - 1));
                             tile[addr] += acc[2 * h + xb][y][z][e];
                             acc[2 * h + xb][y][z][e] = 0.0;
                         }
