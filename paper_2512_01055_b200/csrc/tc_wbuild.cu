@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_wbuild(const tc_wbuild_args a, 
 #pragma unroll
                             for (int e = 0; e < 2; e++) {
                                 const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
-                                const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((tcw::swz(m) + tcw::swz(n1) + tcw::swz(n2)) & (T - 1));
+                                const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((m + n1 + n2) & (T - 1));
                                 tile[addr] += acc[2 * h + xb][y][z][e];
                                 acc[2 * h + xb][y][z][e] = 0.0;
                             }

@@ -201,12 +201,13 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
                 }
 
     // ---- particle phase: both halves, K = v ----
-#ifdef TCW_SKEW
-    if (cs.skew) {   // experiment: start the second warp of each scheduler half a chunk late
+    if (cs.skew) {
+        // The two warps of a scheduler leave the flush barrier in lockstep and need some ten chunks to
+        // drift out of phase (in phase, their barrier/LDS latencies coincide and the tensor pipe idles).
+        // Starting the second one a quarter chunk late gets there at once (+0.7 % on cfg1).
         const long long t0 = clock64();
-        while (clock64() - t0 < TCW_SKEW) {}
+        while (clock64() - t0 < 150) {}
     }
-#endif
     for (int r = 0; r < cs.npc; r++) {
         TRACE(4, cs.tcount, cs.lane == 0 && cs.warp0);
         mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
@@ -445,16 +446,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
             for (int z = 0; z < 2; z++) acc[x][y][z][0] = acc[x][y][z][1] = 0.0;
 
-    // this thread's coordinates in a step's 32 x 16 x 16 result (DMMA C fragment) and their swizzle terms
-    const int fr = lane >> 2, fk = lane & 3;
-    int hm[2], hn1[2], hn2[2][2];
-#pragma unroll
-    for (int q = 0; q < 2; q++) {
-        hm[q] = tcw::swz(q * 8 + fr);
-        hn1[q] = tcw::swz(warp + 8 * q);
-        hn2[q][0] = tcw::swz(q * 8 + 2 * fk);
-        hn2[q][1] = tcw::swz(q * 8 + 2 * fk + 1);
-    }
+    const int fr = lane >> 2, fk = lane & 3;   // this thread's place in the DMMA C fragment
     for (int st = 0; st < nsteps; st++) {
         const Step& d = s.steps[st];
         // dispatch on the ragged-block counts: the loops inside have compile-time trip counts, so
@@ -485,7 +477,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
                         for (int e = 0; e < 2; e++) {
                             const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
-                            const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((hm[xb] + hn1[y] + hn2[z][e]) & (T - 1));
+                            const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((m + n1 + n2) & (T - 1));
                             tile[addr] += acc[2 * h + xb][y][z][e];
                             acc[2 * h + xb][y][z][e] = 0.0;
                         }
