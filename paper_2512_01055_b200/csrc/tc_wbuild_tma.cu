@@ -136,6 +136,9 @@ __device__ __forceinline__ double lds64(uint32_t addr) {
     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(x) : "r"(addr));
     return x;
 }
+__device__ __forceinline__ void sts64(uint32_t addr, double x) {
+    asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(x) : "memory");
+}
 __device__ __forceinline__ void cons_advance(ConsumerState& cs) {
     if (++cs.stage == STAGES) {
         cs.stage = 0;
@@ -447,6 +450,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             for (int z = 0; z < 2; z++) acc[x][y][z][0] = acc[x][y][z][1] = 0.0;
 
     const int fr = lane >> 2, fk = lane & 3;   // this thread's place in the DMMA C fragment
+    const uint32_t tiles0 = opaque(smem_u32(&s.tiles[0]));
     for (int st = 0; st < nsteps; st++) {
         const Step& d = s.steps[st];
         // dispatch on the ragged-block counts: the loops inside have compile-time trip counts, so
@@ -463,13 +467,22 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             default: run_step<1, 1, 1>(acc, cs); break;
         }
         // ---- flush: add the two 16-row halves into their W tiles, permutation in the address ----
+        // (explicit 32-bit shared addresses; per row block 16 loads in flight, then 16 adds and stores)
 #pragma unroll
         for (int h = 0; h < 2; h++) {
-            consumer_bar();  // orders this add after every earlier add to the same element (other steps / other half)
-            double* tile = s.tiles + d.slot[h] * TILE;
+            // Two threads add to the same tile element only from different (step, half) pairs.  Different
+            // steps are ordered by the ring: a warp cannot pass chunk c+STAGES before every warp has released
+            // chunk c, and a warp releases a step's chunks before it flushes the next step, so with at least
+            // STAGES+1 chunks per step the adds of step s happen-before those of step s+1 (through the
+            // empty/full barriers) without any CTA barrier -- the warps keep their phase offsets across steps.
+            // The two halves of one step meet on a tile only when tile indices repeat.
+            if (cps <= STAGES || (h == 1 && d.slot[0] == d.slot[1])) consumer_bar();
+            const uint32_t tile = tiles0 + (uint32_t)d.slot[h] * (TILE * 8);
             const int sm = d.sm[h], sn1 = d.sn1[h], sn2 = d.sn2[h];
 #pragma unroll
-            for (int xb = 0; xb < 2; xb++)
+            for (int xb = 0; xb < 2; xb++) {
+                uint32_t ad[2][2][2];
+                double old[2][2][2];
 #pragma unroll
                 for (int y = 0; y < 2; y++)
 #pragma unroll
@@ -477,10 +490,19 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
                         for (int e = 0; e < 2; e++) {
                             const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
-                            const int addr = m * sm + n1 * sn1 + n2 * sn2 + ((m + n1 + n2) & (T - 1));
-                            tile[addr] += acc[2 * h + xb][y][z][e];
+                            ad[y][z][e] = tile + (uint32_t)(m * sm + n1 * sn1 + n2 * sn2 + ((m + n1 + n2) & (T - 1))) * 8;
+                            old[y][z][e] = lds64(ad[y][z][e]);
+                        }
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int z = 0; z < 2; z++)
+#pragma unroll
+                        for (int e = 0; e < 2; e++) {
+                            sts64(ad[y][z][e], old[y][z][e] + acc[2 * h + xb][y][z][e]);
                             acc[2 * h + xb][y][z][e] = 0.0;
                         }
+            }
         }
     }
     consumer_bar();
