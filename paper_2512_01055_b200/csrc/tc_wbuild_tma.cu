@@ -252,6 +252,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     Smem& s = *reinterpret_cast<Smem*>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int o = a.o, v = a.v;
+    TRACE(0, TRACE_N - 1, tid == 0);   // kernel entry
 
     const int trip = blockIdx.x / a.n_orbits;
     const int orbit = blockIdx.x - trip * a.n_orbits;
@@ -507,6 +508,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     }
     consumer_bar();
 
+    TRACE(1, TRACE_N - 1, tid == 0);   // main loop done, epilogue starts
     if (a.W_debug) tcw::dump_W(s.tiles, s.slot_of_perm, bv, v, a.W_debug, tid, NCONS);
     double sum = tcw::orbit_energy(s.tiles, s.slot_of_perm, bv, occ, a, tid, NCONS);
 #pragma unroll
@@ -518,6 +520,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         for (int w = 0; w < NCONS_WARPS; w++) tot += s.red[w];
         a.partial[(size_t)tr.w * a.n_orbits + orbit] = tot;
     }
+    TRACE(2, TRACE_N - 1, tid == 0);   // unit done
 }
 
 // ---- host: tensor maps -----------------------------------------------------------------------
