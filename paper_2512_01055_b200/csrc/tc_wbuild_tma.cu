@@ -254,8 +254,17 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     const int o = a.o, v = a.v;
     TRACE(0, TRACE_N - 1, tid == 0);   // kernel entry
 
+    // CTA order: tile orbit slow, triplet fast.  CTAs that run together then work on the same orbit for
+    // consecutive triplets (i, j, k), (i, j, k+1), ...: they walk the same step sequence and share the slabs of
+    // the slices I_i and I_j (12 of a unit's 18 slabs) in L2; with the triplet slow and the orbit fast,
+    // neighbours share two tiles and hence only 6 of 18.
+#ifdef TCW_ORBIT_FAST
     const int trip = blockIdx.x / a.n_orbits;
     const int orbit = blockIdx.x - trip * a.n_orbits;
+#else
+    const int orbit = blockIdx.x / a.n_trip;
+    const int trip = blockIdx.x - orbit * a.n_trip;
+#endif
     const int4 tr = a.triplets[trip];
     const int occ[3] = {tr.x, tr.y, tr.z};
     const int4 ob = orbits[orbit];
