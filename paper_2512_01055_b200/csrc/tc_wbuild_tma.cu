@@ -113,7 +113,9 @@ __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" 
 // Timeline instrumentation of one CTA (development builds only).
 constexpr int TRACE_N = 2048;
 __device__ long long g_trace[8][TRACE_N];
+#ifndef TCW_TRACE_CTA
 #define TCW_TRACE_CTA 3000
+#endif
 #define TRACE(row, idx, cond) do { if (blockIdx.x == TCW_TRACE_CTA && (cond) && (idx) < TRACE_N) g_trace[row][idx] = clock64(); } while (0)
 #else
 #define TRACE(row, idx, cond) do { } while (0)
