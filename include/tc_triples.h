@@ -131,8 +131,10 @@ tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v,
                                   double* S_dev, double* E_partial_out);
 
 /* End-to-end variant with HOST inputs: copies the DF factors, amplitudes and orbital
- * energies to the device (cudaMalloc/cudaFree inside; this is the one call that
- * allocates), assembles the integrals, computes E(T), returns it on the host.
+ * energies to the device, assembles the integrals, computes E(T) over triplets
+ * first .. first+count-1, returns it on the host.  This is the one call that allocates
+ * device memory: a single slab (inputs + workspace) owned by the context, kept between
+ * calls, grown when a larger problem arrives and freed by tc_destroy.
  * If bytes_h2d != NULL it receives the bytes copied host->device. */
 tc_status tc_triples_energy_host(tc_ctx* ctx, int o, int v, int naux,
                                  const double* eps_occ, const double* eps_vir,

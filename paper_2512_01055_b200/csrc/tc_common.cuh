@@ -20,6 +20,8 @@ struct tc_ctx {
     cudaEvent_t ev_fork, ev_join;  // fork/join of side_stream against the caller's stream
     cudaEvent_t ev_t0, ev_t1, ev_s0, ev_s1, ev_c0, ev_c1;
     double* pinned;                // a few doubles of pinned host memory for scalar results
+    void* host_slab;               // device slab of tc_triples_energy_host, kept between calls (grow-only)
+    size_t host_slab_bytes;
     tc_stats stats;
     char err[512];
 };

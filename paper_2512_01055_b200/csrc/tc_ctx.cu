@@ -61,6 +61,7 @@ extern "C" tc_status tc_destroy(tc_ctx* ctx) {
     for (int n = 0; n < 8; n++)
         if (evs[n]) cudaEventDestroy(evs[n]);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
+    if (ctx->host_slab) cudaFree(ctx->host_slab);
     free(ctx);
     return TC_OK;
 }

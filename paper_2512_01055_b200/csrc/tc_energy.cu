@@ -415,12 +415,26 @@ extern "C" tc_status tc_triples_energy_host(tc_ctx* ctx, int o, int v, int naux,
     const size_t n[7] = {O, V, O * V, O * O * V * V, X * O * O, X * O * V, X * V * V};
     const double* h[7] = {eps_occ, eps_vir, t1, t2, Boo, Bov, Bvv};
     double* d[7] = {0, 0, 0, 0, 0, 0, 0};
-    void* ws = nullptr;
-    size_t copied = 0;
-    cudaError_t e = cudaMalloc(&ws, wsb);
+    // one device slab for the inputs and the workspace, kept in the context between calls (grow-only):
+    // repeated calls pay for the copies, not for cudaMalloc/cudaFree
+    size_t need = align_up(wsb);
+    for (int q = 0; q < 7; q++) need += align_up(n[q] * sizeof(double));
+    if (need > ctx->host_slab_bytes) {
+        if (ctx->host_slab) cudaFree(ctx->host_slab);
+        ctx->host_slab = nullptr;
+        ctx->host_slab_bytes = 0;
+        cudaError_t ea = cudaMalloc(&ctx->host_slab, need);
+        if (ea != cudaSuccess) TC_FAIL(ctx, TC_ERR_CUDA, "device allocation of %zu bytes failed: %s", need, cudaGetErrorString(ea));
+        ctx->host_slab_bytes = need;
+    }
+    char* slab = (char*)ctx->host_slab;
+    void* ws = slab;
+    size_t off = align_up(wsb), copied = 0;
+    cudaError_t e = cudaSuccess;
     for (int q = 0; q < 7 && e == cudaSuccess; q++) {
-        e = cudaMalloc(&d[q], n[q] * sizeof(double));
-        if (e == cudaSuccess) e = cudaMemcpyAsync(d[q], h[q], n[q] * sizeof(double), cudaMemcpyHostToDevice, 0);
+        d[q] = (double*)(slab + off);
+        off += align_up(n[q] * sizeof(double));
+        e = cudaMemcpyAsync(d[q], h[q], n[q] * sizeof(double), cudaMemcpyHostToDevice, 0);
         copied += n[q] * sizeof(double);
     }
     if (e == cudaSuccess) {
@@ -429,9 +443,7 @@ extern "C" tc_status tc_triples_energy_host(tc_ctx* ctx, int o, int v, int naux,
         st = tc_triples_energy_slice(ctx, o, v, d[0], d[1], d[2], d[3], nullptr, &df, ws, wsb, 0, first, count, nullptr, &E);
         if (st == TC_OK) *E_out = E;
     }
-    for (int q = 0; q < 7; q++) cudaFree(d[q]);
-    cudaFree(ws);
-    if (e != cudaSuccess) TC_FAIL(ctx, TC_ERR_CUDA, "device allocation or copy failed: %s", cudaGetErrorString(e));
+    if (e != cudaSuccess) TC_FAIL(ctx, TC_ERR_CUDA, "host->device copy failed: %s", cudaGetErrorString(e));
     if (st == TC_OK && bytes_h2d) *bytes_h2d = copied;
     return st;
 }

@@ -339,7 +339,6 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     const int nhc = (o + KC - 1) / KC;  // chunks per hole phase
     const int npc = (v + KC - 1) / KC;  // chunks of the particle phase
     const int cps = 2 * nhc + npc;      // chunks per step
-    const int total = nsteps * cps;
 
     if (warp >= NCONS_WARPS) {
         // =========================== producers: four warps, one operand stream each ===========================
