@@ -19,6 +19,8 @@
 // so every fragment load of the 8 consumer warps is one conflict-free 256-byte LDS.64 and the
 // consumers execute only LDS + DMMA (+ one mbarrier wait/arrive per chunk).  Ragged tiles are
 // zero-filled by TMA; 8-blocks that are entirely outside v are neither loaded nor multiplied.
+#include <type_traits>
+
 #include "tc_wbuild_shared.cuh"
 
 namespace {
@@ -131,6 +133,12 @@ struct ConsumerState {
     uint32_t bB, bAp, bAh;   // this thread's fragment addresses in stage 0 (B, particle A, hole A)
     bool warp0, warp5;       // timeline instrumentation: is this consumer warp 0 / 5
     bool skew;               // second warp of its scheduler (warps w and w+4 share one)
+    // deferred flush of the previous step's half 1 (rows 16-31): folded into the W tile under the hole phase of
+    // half 0, whose chunks carry only half the DMMAs and leave the warp idle most of the time
+    bool pend_on;
+    uint32_t pend_tile;      // shared address of the target tile
+    int pend_sm, pend_sn1, pend_sn2;
+    int fr, fk, warp;        // place of this thread in the DMMA C fragment / of its warp in the column tile
 };
 
 __device__ __forceinline__ double lds64(uint32_t addr) {
@@ -163,9 +171,44 @@ __device__ __forceinline__ void cons_release(const ConsumerState& cs, int stage)
 template <int NXB, int NY, int NZ>
 __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerState& cs) {
     constexpr uint32_t BST = B_STAGE * 8, AST = A_STAGE * 8;  // stage strides in bytes
+    // slice Q = (xb, y) of the pending half: the 4 accumulators acc[2+xb][y][z][e] (always full size: blocks a
+    // ragged variant skipped are zero)
+    auto flush_slice = [&](auto qc) {
+        constexpr int Q = decltype(qc)::value;
+        constexpr int xb = Q >> 1, y = Q & 1;
+        uint32_t ad[2][2];
+        double old[2][2];
+#pragma unroll
+        for (int z = 0; z < 2; z++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const int m = xb * 8 + cs.fr, n1 = cs.warp + 8 * y, n2 = z * 8 + 2 * cs.fk + e;
+                ad[z][e] = cs.pend_tile + (uint32_t)(m * cs.pend_sm + n1 * cs.pend_sn1 + n2 * cs.pend_sn2 + ((m + n1 + n2) & (T - 1))) * 8;
+                old[z][e] = lds64(ad[z][e]);
+            }
+#pragma unroll
+        for (int z = 0; z < 2; z++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                sts64(ad[z][e], old[z][e] + acc[2 + xb][y][z][e]);
+                acc[2 + xb][y][z][e] = 0.0;
+            }
+    };
+    auto flush_slice_n = [&](int q) {
+        switch (q) {
+            case 0: flush_slice(std::integral_constant<int, 0>{}); break;
+            case 1: flush_slice(std::integral_constant<int, 1>{}); break;
+            case 2: flush_slice(std::integral_constant<int, 2>{}); break;
+            default: flush_slice(std::integral_constant<int, 3>{}); break;
+        }
+    };
     // ---- hole phases: rows of half h only, K = o ----
 #pragma unroll
     for (int h = 0; h < 2; h++) {
+        if (h == 1 && cs.pend_on) {   // fewer than four hole chunks: finish the pending half before its rows are reused
+            for (int q = cs.nhc; q < 4; q++) flush_slice_n(q);
+            cs.pend_on = false;
+        }
         for (int r = 0; r < cs.nhc; r++) {
             TRACE(4, cs.tcount, cs.lane == 0 && cs.warp0);
             mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
@@ -186,6 +229,7 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
 #pragma unroll
                     for (int z = 0; z < NZ; z++) dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[xb], fb[y][z]);
             cons_release(cs, cs.stage);
+            if (h == 0 && cs.pend_on && r < 4) flush_slice_n(r);
             TRACE(6, cs.tcount, cs.lane == 0 && cs.warp0);
             TRACE(7, cs.tcount, cs.lane == 0 && cs.warp5);
             cs.tcount++;
@@ -440,6 +484,10 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     cs.warp0 = (warp == 0);
     cs.warp5 = (warp == 5);
     cs.skew = (warp & 4) != 0;
+    cs.pend_on = false;
+    cs.fr = lane >> 2;
+    cs.fk = lane & 3;
+    cs.warp = warp;
     cs.nhc = nhc;
     cs.npc = npc;
     cs.full0 = opaque(smem_u32(&s.full[0]));
@@ -479,8 +527,20 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         }
         // ---- flush: add the two 16-row halves into their W tiles, permutation in the address ----
         // (explicit 32-bit shared addresses; per row block 16 loads in flight, then 16 adds and stores)
+        // Half 1 can wait: the next step's first phase (hole, half 0) touches rows 0-15 only, so rows 16-31 are
+        // folded into their tile under it, four accumulators per hole chunk (see run_step).  Not when the two halves
+        // share a tile (they need the barrier between them) and not for very short steps (ring-ordering argument).
+        const bool defer = (cps >= 16) && (d.slot[0] != d.slot[1]);
 #pragma unroll
         for (int h = 0; h < 2; h++) {
+            if (h == 1 && defer) {
+                cs.pend_on = true;
+                cs.pend_tile = tiles0 + (uint32_t)d.slot[1] * (TILE * 8);
+                cs.pend_sm = d.sm[1];
+                cs.pend_sn1 = d.sn1[1];
+                cs.pend_sn2 = d.sn2[1];
+                break;
+            }
             // Two threads add to the same tile element only from different (step, half) pairs.  Different
             // steps are ordered by the ring: a warp cannot pass chunk c+STAGES before every warp has released
             // chunk c, and a warp releases a step's chunks before it flushes the next step, so with at least
@@ -514,6 +574,23 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                             acc[2 * h + xb][y][z][e] = 0.0;
                         }
             }
+        }
+    }
+    if (cs.pend_on) {   // the last step's half 1
+        for (int q = 0; q < 4; q++) {
+            const int xb = q >> 1, y = q & 1;
+#pragma unroll
+            for (int z = 0; z < 2; z++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
+                    const uint32_t ad = cs.pend_tile + (uint32_t)(m * cs.pend_sm + n1 * cs.pend_sn1 + n2 * cs.pend_sn2 + ((m + n1 + n2) & (T - 1))) * 8;
+                    double x = 0.0;
+#pragma unroll
+                    for (int qq = 0; qq < 4; qq++)
+                        if (qq == q) x = acc[2 + (qq >> 1)][qq & 1][z][e];
+                    sts64(ad, lds64(ad) + x);
+                }
         }
     }
     consumer_bar();
