@@ -395,6 +395,12 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
         const int pw = warp - NCONS_WARPS;
         const bool leader = elect_one();
+        if (leader) {   // the descriptors this stream uses: keep their first use off the critical path
+            const CUtensorMap* m0 = (pw < 2) ? &mapI : &mapT2p;
+            const CUtensorMap* m1 = (pw < 2) ? &mapT2h : &mapOvoo;
+            asm volatile("prefetch.tensormap [%0];" ::"l"(m0) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(m1) : "memory");
+        }
         const uint32_t full0 = smem_u32(&s.full[0]), empty0 = smem_u32(&s.empty[0]);
         const uint32_t B0 = smem_u32(&s.B[0][0]), A0 = smem_u32(&s.A[0][0]);
         // A segment = one phase of one step as seen by this stream: n chunks along one K coordinate.
