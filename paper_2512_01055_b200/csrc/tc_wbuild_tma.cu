@@ -12,13 +12,17 @@
 // whose two 16-row halves are added into two W tiles with the index permutation folded into
 // the shared-memory store address (no PERMUTE kernel).
 //
-// Roles: warp 8 (one elected lane) is the TMA producer: per K chunk of 4 it issues
-// cp.async.bulk.tensor boxes that land directly in the fragment order of mma.sync m8n8k4 f64
-//   B stage [z][n1][k][8]  <- box (8 c, 4 d, 16 b) of the slice viewed as dims (c, d, b, slot)
-//   A stage [rowblock][..] <- box (4 d, 16 m) of t2 rows (particle) or (8 m, 4 l) of (ov|oo) (hole)
-// so every fragment load of the 8 consumer warps is one conflict-free 256-byte LDS.64 and the
-// consumers execute only LDS + DMMA (+ one mbarrier wait/arrive per chunk).  Ragged tiles are
-// zero-filled by TMA; 8-blocks that are entirely outside v are neither loaded nor multiplied.
+// Roles (384 threads, 1 CTA per SM, setmaxnreg 40 / 232):
+//   warps 8-11  producers, one operand stream each (B columns 0-7 + expect_tx, B columns 8-15, A half 0, A half 1):
+//               per K chunk of 4 each issues one cp.async.bulk.tensor box into a 3-stage ring; the boxes land
+//               directly in the fragment order of mma.sync m8n8k4 f64
+//                 B stage [z][n1][k][8]  <- box (8 c, 4 d, 16 b) of the slice viewed as dims (c, d, b, slot)
+//                 A stage [rowblock][..] <- box (4 d, 16 m) of t2 rows (particle) or (8 m, 4 l) of (ov|oo) (hole)
+//   warps 0-7   consumers, warp tile 32 x 32: per chunk  wait full -> 8 conflict-free 256-byte LDS.64 ->
+//               16 DMMA.8x8x4 -> release; after a step they add their accumulators into the W tiles
+//               (half 0 at once, half 1 under the next step's half-0 hole phase), at the end they run the epilogue.
+// Ragged tiles are zero-filled by TMA; 8-blocks that are entirely outside v are neither loaded nor multiplied.
+// CTA order: tile orbit slow, triplet fast (L2 reuse of the I_i and I_j slabs between concurrent CTAs).
 #include <type_traits>
 
 #include "tc_wbuild_shared.cuh"
