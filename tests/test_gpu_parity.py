@@ -215,3 +215,21 @@ def test_argument_errors(ctx):
     with pytest.raises(TcError):   # host pointer where a device pointer is required
         ctx.triples_energy(p.o, p.v, p.eps_occ.ctypes.data, dp.eps_vir, dp.t1, dp.t2, blocks=dp.blocks(), workspace=ws,
                            workspace_bytes=ws.numel())
+
+
+def test_empty_range_and_fallback_kernel_on_even_v(ctx, monkeypatch):
+    """count = 0 is a valid (empty) range; the cp.async fallback kernel (used for odd v) gives the same numbers as the
+    TMA kernel on an even-v problem (TC_FORCE_CPASYNC is a testing aid of the library)."""
+    p = synth.make_problem(4, 24, 6, 9, sigma_B=0.25, blocks=True)
+    dp = DevProblem(p)
+    n = oracle.triplet_count(p.o)
+    E0, _ = run_slice(ctx, dp, 3, 0)
+    assert E0 == 0.0
+    E_ref, S_ref = oracle.triples_energy(p)
+    E_tma, S_tma = run_slice(ctx, dp, 0, n)
+    monkeypatch.setenv("TC_FORCE_CPASYNC", "1")
+    E_cp, S_cp = run_slice(ctx, dp, 0, n)
+    monkeypatch.delenv("TC_FORCE_CPASYNC")
+    for E, S in ((E_tma, S_tma), (E_cp, S_cp)):
+        assert np.abs(S - S_ref).max() <= REL_TOL * np.abs(S_ref).max()
+        assert_energy(E, E_ref)
