@@ -190,11 +190,12 @@ extern "C" tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v, const do
         if (st != TC_OK) return st;
         // slices land at an aligned stride so each starts on a 256-byte boundary
         slice_stride = align_up(sizeof(double) * (size_t)v * v * v) / sizeof(double);
-        for (int x = 0; x < o && L.n_slots >= o; x++) {
-            TC_CUDA(ctx, tc_launch_df_gemm(df->Bvv, (size_t)v * v, df->Bov + (size_t)x * v, (size_t)o * v, v * v, v, df->naux, 1,
-                                           (long long)v, 0, v, 0, 1, w_vvvo + (size_t)x * slice_stride, s));
+        if (L.n_slots >= o) {
+            // all o slices in one launch: column (x, c) of the v^2 x (o v) product lands at x * slice_stride + c
+            TC_CUDA(ctx, tc_launch_df_gemm(df->Bvv, (size_t)v * v, df->Bov, (size_t)o * v, v * v, o * v, df->naux, 1, (long long)v, 0,
+                                           v, (long long)slice_stride, 1, w_vvvo, s));
             ctx->stats.n_kernel_launches++;
-            ctx->stats.slices_built++;
+            ctx->stats.slices_built += o;
         }
         TC_CUDA(ctx, cudaEventRecord(ctx->ev_s1, s));
         ovoo = w_ovoo;
