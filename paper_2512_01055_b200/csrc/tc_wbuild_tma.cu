@@ -142,6 +142,10 @@ struct ConsumerState {
     bool pend_on;
     uint32_t pend_tile;      // shared address of the target tile
     int pend_sm, pend_sn1, pend_sn2;
+    // ... and of its half 0, parked in spare registers (`hold`) and folded in under the hole phase of half 1
+    bool pend0_on;
+    uint32_t pend0_tile;
+    int pend0_sm, pend0_sn1, pend0_sn2;
     int fr, fk, warp;        // place of this thread in the DMMA C fragment / of its warp in the column tile
 };
 
@@ -173,7 +177,7 @@ __device__ __forceinline__ void cons_release(const ConsumerState& cs, int stage)
 // this shape measures 99 % of the DMMA peak, with the mbarrier ring and TMA producers 91 %;
 // DESIGN.md "what the consumer loop can reach").
 template <int NXB, int NY, int NZ>
-__device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerState& cs) {
+__device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], double (&hold)[2][2][2][2], ConsumerState& cs) {
     constexpr uint32_t BST = B_STAGE * 8, AST = A_STAGE * 8;  // stage strides in bytes
     // slice Q = (xb, y) of the pending half: the 4 accumulators acc[2+xb][y][z][e] (always full size: blocks a
     // ragged variant skipped are zero)
@@ -197,6 +201,26 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
                 sts64(ad[z][e], old[z][e] + acc[2 + xb][y][z][e]);
                 acc[2 + xb][y][z][e] = 0.0;
             }
+    };
+    auto flush_hold_slice = [&](auto qc) {
+        constexpr int Q = decltype(qc)::value;
+        constexpr int xb = Q >> 1, y = Q & 1;
+#pragma unroll
+        for (int z = 0; z < 2; z++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const int m = xb * 8 + cs.fr, n1 = cs.warp + 8 * y, n2 = z * 8 + 2 * cs.fk + e;
+                const uint32_t ad = cs.pend0_tile + (uint32_t)(m * cs.pend0_sm + n1 * cs.pend0_sn1 + n2 * cs.pend0_sn2 + ((m + n1 + n2) & (T - 1))) * 8;
+                sts64(ad, lds64(ad) + hold[xb][y][z][e]);
+            }
+    };
+    auto flush_hold_n = [&](int q) {
+        switch (q) {
+            case 0: flush_hold_slice(std::integral_constant<int, 0>{}); break;
+            case 1: flush_hold_slice(std::integral_constant<int, 1>{}); break;
+            case 2: flush_hold_slice(std::integral_constant<int, 2>{}); break;
+            default: flush_hold_slice(std::integral_constant<int, 3>{}); break;
+        }
     };
     auto flush_slice_n = [&](int q) {
         switch (q) {
@@ -234,11 +258,16 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
                     for (int z = 0; z < NZ; z++) dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[xb], fb[y][z]);
             cons_release(cs, cs.stage);
             if (h == 0 && cs.pend_on && r < 4) flush_slice_n(r);
+            if (h == 1 && cs.pend0_on && r < 4) flush_hold_n(r);
             TRACE(6, cs.tcount, cs.lane == 0 && cs.warp0);
             TRACE(7, cs.tcount, cs.lane == 0 && cs.warp5);
             cs.tcount++;
             cons_advance(cs);
         }
+    }
+    if (cs.pend0_on) {   // fewer than four hole chunks: the rest of the parked half 0
+        for (int q = cs.nhc; q < 4; q++) flush_hold_n(q);
+        cs.pend0_on = false;
     }
     // the hole sums enter W with a minus sign (eq. (2))
 #pragma unroll
@@ -495,6 +524,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     cs.warp5 = (warp == 5);
     cs.skew = (warp & 4) != 0;
     cs.pend_on = false;
+    cs.pend0_on = false;
     cs.fr = lane >> 2;
     cs.fk = lane & 3;
     cs.warp = warp;
@@ -520,20 +550,21 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 
     const int fr = lane >> 2, fk = lane & 3;   // this thread's place in the DMMA C fragment
     const uint32_t tiles0 = opaque(smem_u32(&s.tiles[0]));
+    double hold[2][2][2][2];   // half 0 of the previous step while it waits for the hole phase of half 1
     for (int st = 0; st < nsteps; st++) {
         const Step& d = s.steps[st];
         // dispatch on the ragged-block counts: the loops inside have compile-time trip counts, so
         // the DMMAs carry no predicates (predicated mma.sync costs a WARPSYNC + NOP each)
         const int code = (d.nxb - 1) * 4 + (d.ny - 1) * 2 + (d.nz - 1);
         switch (code) {
-            case 7: run_step<2, 2, 2>(acc, cs); break;
-            case 6: run_step<2, 2, 1>(acc, cs); break;
-            case 5: run_step<2, 1, 2>(acc, cs); break;
-            case 4: run_step<2, 1, 1>(acc, cs); break;
-            case 3: run_step<1, 2, 2>(acc, cs); break;
-            case 2: run_step<1, 2, 1>(acc, cs); break;
-            case 1: run_step<1, 1, 2>(acc, cs); break;
-            default: run_step<1, 1, 1>(acc, cs); break;
+            case 7: run_step<2, 2, 2>(acc, hold, cs); break;
+            case 6: run_step<2, 2, 1>(acc, hold, cs); break;
+            case 5: run_step<2, 1, 2>(acc, hold, cs); break;
+            case 4: run_step<2, 1, 1>(acc, hold, cs); break;
+            case 3: run_step<1, 2, 2>(acc, hold, cs); break;
+            case 2: run_step<1, 2, 1>(acc, hold, cs); break;
+            case 1: run_step<1, 1, 2>(acc, hold, cs); break;
+            default: run_step<1, 1, 1>(acc, hold, cs); break;
         }
         // ---- flush: add the two 16-row halves into their W tiles, permutation in the address ----
         // (explicit 32-bit shared addresses; per row block 16 loads in flight, then 16 adds and stores)
@@ -541,8 +572,27 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         // folded into their tile under it, four accumulators per hole chunk (see run_step).  Not when the two halves
         // share a tile (they need the barrier between them) and not for very short steps (ring-ordering argument).
         const bool defer = (cps >= 16) && (d.slot[0] != d.slot[1]);
+        if (defer) {   // park half 0 in spare registers: nothing of the flush is left on the critical path
+#pragma unroll
+            for (int xb = 0; xb < 2; xb++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int z = 0; z < 2; z++)
+#pragma unroll
+                        for (int e = 0; e < 2; e++) {
+                            hold[xb][y][z][e] = acc[xb][y][z][e];
+                            acc[xb][y][z][e] = 0.0;
+                        }
+            cs.pend0_on = true;
+            cs.pend0_tile = tiles0 + (uint32_t)d.slot[0] * (TILE * 8);
+            cs.pend0_sm = d.sm[0];
+            cs.pend0_sn1 = d.sn1[0];
+            cs.pend0_sn2 = d.sn2[0];
+        }
 #pragma unroll
         for (int h = 0; h < 2; h++) {
+            if (h == 0 && defer) continue;
             if (h == 1 && defer) {
                 cs.pend_on = true;
                 cs.pend_tile = tiles0 + (uint32_t)d.slot[1] * (TILE * 8);
@@ -585,6 +635,20 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                         }
             }
         }
+    }
+    if (cs.pend0_on) {   // the last step's half 0
+#pragma unroll
+        for (int xb = 0; xb < 2; xb++)
+#pragma unroll
+            for (int y = 0; y < 2; y++)
+#pragma unroll
+                for (int z = 0; z < 2; z++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                        const int m = xb * 8 + fr, n1 = warp + 8 * y, n2 = z * 8 + 2 * fk + e;
+                        const uint32_t ad = cs.pend0_tile + (uint32_t)(m * cs.pend0_sm + n1 * cs.pend0_sn1 + n2 * cs.pend0_sn2 + ((m + n1 + n2) & (T - 1))) * 8;
+                        sts64(ad, lds64(ad) + hold[xb][y][z][e]);
+                    }
     }
     if (cs.pend_on) {   // the last step's half 1
         for (int q = 0; q < 4; q++) {
