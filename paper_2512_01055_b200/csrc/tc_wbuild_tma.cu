@@ -20,7 +20,8 @@
 //                 A stage [rowblock][..] <- box (4 d, 16 m) of t2 rows (particle) or (8 m, 4 l) of (ov|oo) (hole)
 //   warps 0-7   consumers, warp tile 32 x 32: per chunk  wait full -> 8 conflict-free 256-byte LDS.64 ->
 //               16 DMMA.8x8x4 -> release; after a step they add their accumulators into the W tiles
-//               (half 0 at once, half 1 under the next step's half-0 hole phase), at the end they run the epilogue.
+//               under the next step's hole phases (half 1 from its accumulators, half 0 from spare registers),
+//               at the end they run the epilogue.
 // Ragged tiles are zero-filled by TMA; 8-blocks that are entirely outside v are neither loaded nor multiplied.
 // CTA order: tile orbit slow, triplet fast (L2 reuse of the I_i and I_j slabs between concurrent CTAs).
 #include <type_traits>
