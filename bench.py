@@ -251,8 +251,8 @@ def run_ours(args):
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
-    # DRAM bytes of one k_wbuild_tma launch from ncu (profiles/r01d_final_kernel.md): measured on the full cfg1 range
-    traffic = 207904411136 + 3579982592 if (args.config == "cfg1" and world == 1 and count == ntrip) else None
+    # DRAM bytes of one k_wbuild_tma launch from ncu (profiles/r01e_committed_kernel.md): measured on the full cfg1 range
+    traffic = 216451098880 + 3586434304 if (args.config == "cfg1" and world == 1 and count == ntrip) else None
     roofline = {"bound": "tensor", "kernel": "k_wbuild_tma", "achieved": achieved, "peak": dmma_sus, "unit": UNIT,
                 "frac": achieved / dmma_sus, "traffic": traffic, "traffic_unit": "bytes per launch (dram read+write, ncu)",
                 "peak_source": "FP64 DMMA.8x8x4 microbenchmark measured in this run (sustained 2 s); "
