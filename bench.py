@@ -4,11 +4,15 @@
 A "step" is one pass of the whole hot path over one synthetic
 problem: tc_triples_energy with DF-factor input, i.e. triplet scheduling, DF -> integral-block
 assembly, the fused W contractions + on-chip epilogue, and the reductions.  Default workload:
-BASELINE.json configs[1] (o=20, v=200, naux=600, seed 1), inputs resident in HBM.
+BASELINE.json configs[1] (o=20, v=200, naux=600, seed 1), the full problem, inputs resident in HBM.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg1] [--impl ours|reference]
 
-N > 1 (torchrun): the linear triplet index is partitioned into N contiguous ranges, one per
+Besides the timed steps the default run measures, once each and outside the timed loop, a triplet slice of every
+other BASELINE config (cfg2, cfg3, cfg4 through the slice cache), of the paper's own shape (h2o14: o=70, v=266) and of an
+odd-v twin of cfg1 -- the `configs` block -- and the roofline denominators (DMMA / DFMA / ring / copy microbenchmarks).
+
+N > 1 (torchrun): the linear triplet index is partitioned into N contiguous ranges (tc_triplet_partition), one per
 rank; the only exchange is one all-reduce of the FP64 partial energy.  `value` is whole-job
 TFLOP/s = executed contraction flop of all ranks / max-over-ranks device time.
 
@@ -18,6 +22,7 @@ triplet sample of the same workload.
 from __future__ import annotations
 
 import argparse
+import glob
 import json
 import os
 import subprocess
@@ -38,18 +43,6 @@ def flops_per_triplet(o, v):
     return 12.0 * v ** 3 * (v + o)
 
 
-def nonzero_in_range(o, first, count):
-    from paper_2512_01055_b200 import binding
-    return sum(1 for n in range(first, first + count) if binding.triplet_decode(o, n)[3] != 0.0)
-
-
-def partition(ntrip, world, rank):
-    """Contiguous range of the linear triplet index owned by `rank` (sizes differ by at most one)."""
-    base, rem = divmod(ntrip, world)
-    first = rank * base + min(rank, rem)
-    return first, base + (1 if rank < rem else 0)
-
-
 class ClockSampler:
     """nvidia-smi SM clock / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
 
@@ -66,6 +59,7 @@ class ClockSampler:
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
             self.proc = None
+        return self
 
     def _read(self):
         for line in self.proc.stdout:
@@ -88,6 +82,7 @@ class ClockSampler:
 def oracle_sample(prob_cfg, seconds_target=15.0):
     """Time the CPU oracle on a bounded triplet sample of the workload; returns a cpu_baseline dict."""
     import oracle
+    from oracle import blocks as oblocks
     from paper_2512_01055_b200 import synth
     o, v, naux, seed = synth.config_sizes(prob_cfg)
     p = synth.make_config(prob_cfg)
@@ -95,10 +90,9 @@ def oracle_sample(prob_cfg, seconds_target=15.0):
     ntrip = oracle.triplet_count(o)
     first = ntrip - 1
     i, j, k, _ = oracle.triplet_decode(o, first)
-    slices = {x: synth.vvvo_slice(p, x) for x in {i, j, k}}
-    if p.ovoo is None:
-        p.ovoo = np.ascontiguousarray(np.einsum("qlj,qkc->jklc", p.Boo, p.Bov, optimize=True))
-        p.ovov = np.ascontiguousarray(np.einsum("qjb,qkc->jkbc", p.Bov, p.Bov, optimize=True))
+    slices = {x: oblocks.vvvo_slice(p, x) for x in {i, j, k}}
+    p.ovoo = oblocks.ovoo_block(p)
+    p.ovov = oblocks.ovov_block(p)
     t0 = time.perf_counter()
     oracle.triples_energy_slices(p, slices, first, 1)
     t1 = time.perf_counter() - t0
@@ -108,7 +102,7 @@ def oracle_sample(prob_cfg, seconds_target=15.0):
     need = set()
     for q in range(first, ntrip):
         need.update(oracle.triplet_decode(o, q)[:3])
-    slices = {x: slices[x] if x in slices else synth.vvvo_slice(p, x) for x in need}
+    slices = {x: slices[x] if x in slices else oblocks.vvvo_slice(p, x) for x in need}
     t0 = time.perf_counter()
     oracle.triples_energy_slices(p, slices, first, n)
     dt = time.perf_counter() - t0
@@ -145,6 +139,64 @@ def run_reference(args):
     }))
 
 
+def newest_traffic():
+    """DRAM bytes of one k_wbuild_tma launch over the full cfg1 range, from the newest ncu capture committed under
+    profiles/ (rXX*_traffic_full_launch.csv, ncu --csv; the .md beside it names the command).  None if none parses."""
+    import csv
+    units = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic_full_launch.csv"))):
+        got = {}
+        try:
+            rows = [r for r in csv.reader(l for l in open(path) if l.startswith('"'))]
+            head = rows[0]
+            i_name, i_unit, i_val, i_kern = (head.index(k) for k in ("Metric Name", "Metric Unit", "Metric Value", "Kernel Name"))
+            for r in rows[1:]:
+                if "k_wbuild_tma" in r[i_kern] and r[i_name] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                    got[r[i_name]] = float(r[i_val].replace(",", "")) * units.get(r[i_unit], 1.0)
+        except Exception:
+            continue
+        if len(got) == 2:
+            best = {"bytes": sum(got.values()), "source": os.path.relpath(path, ROOT)}
+    return best
+
+
+def measure_slice(ctx, torch, synth, name, first, count, dmma_peak, reps=2):
+    """One triplet slice of another config, DF input, timed by the library's own CUDA events (whole call)."""
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    o, v, naux, seed = synth.config_sizes(name)
+    t_gen = time.perf_counter()
+    d = synth.make_problem_device(o, v, naux, seed)
+    torch.cuda.synchronize()
+    t_gen = time.perf_counter() - t_gen
+    free_b = torch.cuda.mem_get_info()[0] - (3 << 30)
+    nb = ctx.workspace_bytes(o, v, naux, free_b)
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    df = (naux, d["Boo"], d["Bov"], d["Bvv"])
+    best = None
+    sampler = ClockSampler(torch.cuda.current_device()).start()
+    for _ in range(reps):
+        E = ctx.triples_energy_slice(o, v, d["eps_occ"], d["eps_vir"], d["t1"], d["t2"], df=df, workspace=ws,
+                                     workspace_bytes=nb, first=first, count=count)
+        st = ctx.get_stats()
+        if best is None or st["ms_total"] < best["ms_total"]:
+            best = st
+    clocks = sampler.stop()
+    tf = best["flop_contraction"] / (best["ms_total"] * 1e-3) * 1e-12
+    tfk = best["flop_contraction"] / (max(best["ms_kernels"], 1e-9) * 1e-3) * 1e-12
+    out = {"workload": f"{name}: o={o}, v={v}, naux={naux}, seed {seed}, triplets [{first},{first + count})", "tflops": tf,
+           "frac_of_dmma_peak": tf / dmma_peak, "kernel_tflops": tfk, "kernel_frac": tfk / dmma_peak, "ms_total": best["ms_total"],
+           "ms_kernels": best["ms_kernels"], "ms_staging": best["ms_staging"], "slices_built": best["slices_built"],
+           "n_blocks": best["n_blocks"], "kernel": {1: "k_wbuild_tma", 2: "k_wbuild (cp.async)"}.get(best["kernel"]),
+           "padded": best["padded"], "staging_interval_ms": [best["staging_first_ms"], best["staging_last_ms"]],
+           "contraction_interval_ms": [best["contraction_first_ms"], best["contraction_last_ms"]],
+           "E_partial": E, "input_generation_s": t_gen, "clocks": clocks}
+    del ws, d
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -159,7 +211,7 @@ def run_ours(args):
     ctx = binding.Context(local)
     o, v, naux, seed = synth.config_sizes(args.config)
     ntrip = binding.triplet_count(o)
-    first, count = partition(ntrip, world, rank)
+    first, count = binding.triplet_partition(o, world, rank)   # triplet ranges per rank, behind the C-ABI
     if args.config == "cfg4" and world == 1 and not args.triplets and args.first < 0:
         first, count = 59640, 2000      # BASELINE.json configs[4]: a fixed contiguous slice of 2000 triplets (reading 14)
     if args.first >= 0:
@@ -169,17 +221,15 @@ def run_ours(args):
         count = min(count, args.triplets)
 
     # ---- inputs: seeded, synthetic, generated on the host, resident in HBM before timing ----
-    # (problems whose t2 exceeds 8 GB derive the MP2 amplitudes from the uploaded B_ov on the device)
+    # (problems whose t2 exceeds 8 GB draw the factors and derive the MP2 amplitudes on the device)
     big = 8.0 * o * o * v * v > 8e9
-    p = synth.make_config(args.config, with_t2=not big)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    names = ("eps_occ", "eps_vir", "t1", "Boo", "Bov", "Bvv") + (() if big else ("t2",))
     if big:
         host = {}
-        d = {k: torch.from_numpy(np.ascontiguousarray(getattr(p, k))).cuda() for k in names}
-        d["t2"] = synth.mp2_amplitudes_device(d["Bov"], d["eps_occ"], d["eps_vir"])
+        d = synth.make_problem_device(o, v, naux, seed)
     else:
-        host = {k: pin(getattr(p, k)) for k in names}
+        p = synth.make_config(args.config)
+        host = {k: pin(getattr(p, k)) for k in ("eps_occ", "eps_vir", "t1", "Boo", "Bov", "Bvv", "t2")}
         d = {k: t.cuda(non_blocking=True) for k, t in host.items()}
     torch.cuda.synchronize()
     # workspace: everything the library needs; if all (vv|vo) slices do not fit it sizes a slice cache instead
@@ -205,12 +255,12 @@ def run_ours(args):
     if rank == 0:
         sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ms_contr, launches = [], 0
+    ms_kern, launches = [], 0
     e0.record()
     for _ in range(args.steps):
         E = step()
         st = ctx.get_stats()
-        ms_contr.append(st["ms_contraction"])
+        ms_kern.append(st["ms_kernels"])          # CUDA events around each k_wbuild_tma launch, on the launching stream
         launches += st["n_kernel_launches"]
     e1.record()
     barrier()
@@ -224,14 +274,18 @@ def run_ours(args):
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
         dist.all_reduce(ftot, op=dist.ReduceOp.SUM)   # whole-job flop and the one scalar the method exchanges: E
     ms_all, flop_all, E_all = float(tmax[0]), float(ftot[0]), float(ftot[1])
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()                  # on every rank
+    if rank != 0:
+        return
 
     # ---- end to end through the host-pointer C-ABI call (H2D copies inside the timed region) ----
     e2e = None
+    streamed = None
     if world == 1 and not args.no_e2e and not big:
         hb = [host[k].numpy() for k in ("eps_occ", "eps_vir", "t1", "t2", "Boo", "Bov", "Bvv")]
-        del ws
-        torch.cuda.empty_cache()
-        ctx.triples_energy_host(o, v, naux, *hb, first=first, count=count)   # warm-up
+        ctx.triples_energy_host(o, v, naux, *hb, first=first, count=count)   # warm-up (allocates the context's slab)
         n_e2e = max(1, min(args.steps, 3))
         t0 = time.perf_counter()
         for _ in range(n_e2e):
@@ -239,26 +293,85 @@ def run_ours(args):
         dt = (time.perf_counter() - t0) / n_e2e
         e2e = {"value": flop / dt * 1e-12, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": 8,
                "ms_per_step": dt * 1e3, "E": E_h}
+        # NEXT-3: amplitudes resident on the HOST (pinned), rows streamed through a device ring of o/2 slots on the side
+        # stream under the contractions; everything else as in the timed step
+        try:
+            full_s = ctx.workspace_bytes_streamed(o, v, naux)
+            ldv = v + (v % 2)
+            per_slot = (v * v * ldv * 8 + 255) // 256 * 256 + (o * v * ldv * 8 + 255) // 256 * 256
+            nb_s = ctx.workspace_bytes_streamed(o, v, naux, full_s - (o - max(3, o // 2)) * per_slot)
+            ws_s = ws[:nb_s] if nb_s <= nb else torch.empty(nb_s, dtype=torch.uint8, device="cuda")
+            best = None
+            for _ in range(2):
+                t0 = time.perf_counter()
+                E_s = ctx.triples_energy_streamed(o, v, d["eps_occ"], d["eps_vir"], d["t1"], host["t2"], df=df, workspace=ws_s,
+                                                  workspace_bytes=nb_s, first=first, count=count)
+                dt = time.perf_counter() - t0
+                s2 = ctx.get_stats()
+                if best is None or dt < best[0]:
+                    best = (dt, s2)
+            dt, s2 = best
+            streamed = {"value": flop / dt * 1e-12, "unit": UNIT, "ms_per_step": dt * 1e3, "slots": max(3, o // 2),
+                        "h2d_bytes_per_step": s2["bytes_h2d"], "t2_rows_copied": s2["t2_rows_copied"], "slices_built": s2["slices_built"],
+                        "n_blocks": s2["n_blocks"], "E": E_s, "rel_diff_vs_resident": abs(E_s - E) / abs(E) if E else None}
+        except Exception as ex:   # reported, never hidden
+            streamed = {"error": repr(ex)}
 
-    if rank != 0:
-        return
     # ---- roofline of the dominant kernel (fused W-builder): FP64 tensor pipe ----
     dmma_sus, dmma_burst = ctx.bench_dmma_peak(2.0)
-    ms_k = float(np.mean(ms_contr))
+    ms_k = float(np.mean(ms_kern))
     achieved = flop / (ms_k * 1e-3) * 1e-12
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
-    # DRAM bytes of one k_wbuild_tma launch from ncu (profiles/r01e_committed_kernel.md): measured on the full cfg1 range
-    traffic = 216451098880 + 3586434304 if (args.config == "cfg1" and world == 1 and count == ntrip) else None
+    full_cfg1 = args.config == "cfg1" and world == 1 and count == ntrip
+    tr = newest_traffic() if full_cfg1 else None
     roofline = {"bound": "tensor", "kernel": "k_wbuild_tma", "achieved": achieved, "peak": dmma_sus, "unit": UNIT,
-                "frac": achieved / dmma_sus, "traffic": traffic, "traffic_unit": "bytes per launch (dram read+write, ncu)",
+                "frac": achieved / dmma_sus, "traffic": tr["bytes"] if tr else None,
+                "traffic_unit": "bytes per launch (dram read+write, ncu)", "traffic_source": tr["source"] if tr else None,
                 "peak_source": "FP64 DMMA.8x8x4 microbenchmark measured in this run (sustained 2 s); "
                                f"burst {dmma_burst:.2f}; MEASURED_PEAKS.json has no FP64 figure "
                                f"(bf16 {peaks.get('bf16_tflops')} TF/s, hbm {peaks.get('hbm_gbs')} GB/s)",
-                "kernel_ms_per_step": ms_k}
+                "kernel_ms_per_step": ms_k, "kernel_timing": "CUDA events around each k_wbuild_tma launch on the launching stream"}
+    # the other denominators (north_star: DMMA and copy microbenchmarks) and what the consumer loop can reach
+    micro = None
+    if not args.no_micro:
+        dfma_sus, dfma_burst = ctx.bench_dfma_peak(1.0)
+        nbytes = 1 << 30
+        buf = torch.empty(2 * nbytes, dtype=torch.uint8, device="cuda")
+        copy_gbs = ctx.bench_copy_bw(buf[nbytes:], buf[:nbytes], nbytes, 10)
+        ring = [ctx.bench_ring_peak(q, 0.5, buf, 2 * nbytes) for q in range(3)]
+        del buf
+        micro = {"dmma_tflops": dmma_sus, "dmma_burst_tflops": dmma_burst, "dfma_tflops": dfma_sus, "copy_gbs": copy_gbs,
+                 "copy_gbs_driver": peaks.get("hbm_gbs"),
+                 "ring_tflops": {"lds_dmma": ring[0], "mbarrier_ring": ring[1], "tma_ring": ring[2]},
+                 "ring_frac_of_dmma": [r / dmma_sus for r in ring],
+                 "staging_gbs_equiv": None}
+    golden = None
+    if full_cfg1:
+        try:
+            sys.path.insert(0, os.path.join(ROOT, "tests"))
+            import harness
+            _, E_gold = harness.read_golden_S("cfg1")
+            golden = {"E_oracle": E_gold, "abs_diff": abs(E_all - E_gold), "rel_diff": abs(E_all - E_gold) / abs(E_gold),
+                      "source": "tests/golden/S_cfg1.txt (CPU oracle, full range)"}
+        except Exception as ex:
+            golden = {"error": repr(ex)}
+    # ---- the other configs, one triplet slice each, outside the timed loop ----
+    configs = None
+    if world == 1 and not args.no_configs and args.config == "cfg1":
+        del ws
+        configs = {}
+        plan = [("cfg2", 5000, 296), ("cfg3", 20000, 100), ("h2o14", 30000, 592), ("20,201,600,1", 0, 1540)]
+        if torch.cuda.mem_get_info()[1] > 170e9:
+            plan.append(("cfg4", 59640, 48))
+        for name, f0, cnt in plan:
+            try:
+                configs[name] = measure_slice(ctx, torch, synth, name, f0, cnt, dmma_sus)
+            except Exception as ex:
+                configs[name] = {"error": repr(ex)}
     cb = None if args.no_cpu else oracle_sample(args.config)
     out = {
         "metric": METRIC, "value": flop_all / (ms_all * 1e-3) * 1e-12, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -268,13 +381,12 @@ def run_ours(args):
                                f"triplets [{first},{first + count}) of {ntrip} per rank-0, DF-factor input (a2 staging inside the step)",
                    "l2": "inputs larger than L2 (vvvo %.2f GB vs 126 MB); no explicit flush" % (o * v ** 3 * 8e-9),
                    "parallelism": f"triplet ranges x{world}"},
-        "E_T": E_all, "frac_of_dmma_peak": flop_all / (ms_all * 1e-3) * 1e-12 / (dmma_sus * world),
+        "E_T": E_all, "golden": golden, "frac_of_dmma_peak": flop_all / (ms_all * 1e-3) * 1e-12 / (dmma_sus * world),
         "staging": {"ms_per_step": st["ms_staging"], "slices_built_per_step": st["slices_built"]},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cb,
+        "clocks": clocks, "e2e": e2e, "e2e_t2_on_host": streamed, "gpu_launches": int(launches), "roofline": roofline,
+        "microbenchmarks": micro, "configs": configs, "cpu_baseline": cb,
     }
     print(json.dumps(out))
-    if world > 1:
-        dist.destroy_process_group()
 
 
 def main():
@@ -288,6 +400,8 @@ def main():
     ap.add_argument("--first", type=int, default=-1, help="first triplet of the range (linear index)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the slices of the other configs")
+    ap.add_argument("--no-micro", action="store_true", help="skip the DFMA / copy / ring microbenchmarks")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

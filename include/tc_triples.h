@@ -24,9 +24,13 @@
  *     call returns.  "host" pointers are ordinary host memory.
  *   - All arrays are FP64 ("double"), dense, C order (last index fastest).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
- *     Work is enqueued on it; side streams the library owns are forked from and joined
- *     to it with events, so the caller sees single-stream semantics.  Calls that
- *     return a host scalar synchronise `stream` once before returning.
+ *     Work is enqueued on it.  When the (vv|vo) slices (or, for the streamed call, the
+ *     amplitudes) do not all fit in the workspace, the library runs a blocked schedule
+ *     and stages the operands of the next block on a side stream it owns while the
+ *     current block's contraction runs on `stream`; that side stream is forked from and
+ *     joined to `stream` with events, so the caller sees single-stream semantics.  In
+ *     every other case all work is on `stream` itself.  Calls that return a host scalar
+ *     synchronise `stream` once before returning.
  *   - The library performs no device allocation inside the compute calls: scratch
  *     space is the caller-allocated `workspace` (the paper's "pre-allocate and reuse"
  *     rule).  tc_workspace_bytes tells how much is needed.
@@ -86,6 +90,12 @@ long long tc_triplet_count(int o);
 tc_status tc_triplet_decode(int o, long long idx, int* i, int* j, int* k, double* weight);
 /* (i,j,k), i>=j>=k -> idx, or -1 if the arguments are not an ordered triplet below o. */
 long long tc_triplet_index(int o, int i, int j, int k);
+/* Multi-GPU sharding (the paper hands independent tile batches to the GPUs and sums the partial
+ * energies): the contiguous range [first, first+count) of the linear triplet index
+ * owned by `rank` of `world`.  The ranges tile [0, N_trip) and differ in size by at most one; each
+ * rank runs tc_triples_energy_slice on its range with replicated inputs and the partial energies are
+ * summed (one scalar all-reduce).  Host only. */
+tc_status tc_triplet_partition(int o, int world, int rank, long long* first, long long* count);
 
 /* ---- workspace ------------------------------------------------------------------ */
 
@@ -96,6 +106,25 @@ long long tc_triplet_index(int o, int i, int j, int k);
  *                 budget, else it sizes an LRU cache of per-occupied-index slices.
  * Returns TC_ERR_WORKSPACE_TOO_SMALL if even the minimum does not fit the budget. */
 tc_status tc_workspace_bytes(tc_ctx* ctx, int o, int v, int naux_or_0, size_t hbm_budget, size_t* bytes);
+
+/* The same for tc_triples_energy_streamed (t2 stays on the host; DF input only). */
+tc_status tc_workspace_bytes_streamed(tc_ctx* ctx, int o, int v, int naux, size_t hbm_budget, size_t* bytes);
+
+/* The blocked schedule (what the library does when the per-occupied-index operands -- (vv|v.) slices,
+ * amplitude rows -- are cached in `nslots` < o slots): the triplets are cut into blocks of bi x bj x bk occupied
+ * indices, the operands of a block are made resident (LRU eviction), and the next block's missing operands are
+ * staged while the current block computes.  This host-only call reports the plan for a triplet range:
+ * number of blocks (= W-builder launches), operand loads (slice assemblies), and the block shape chosen.
+ * Any output pointer may be NULL.  Returns TC_ERR_INVALID_ARG if nslots < 3 (a triplet needs three slices). */
+tc_status tc_plan_summary(int o, long long first, long long count, int nslots,
+                          long long* n_blocks, long long* n_loads, int* bi, int* bj, int* bk);
+
+/* The plan itself, for validation (host only): recs_out[count][8] = (i, j, k, index of the triplet in the range,
+ * block, slot of i, slot of j, slot of k) in execution order; loads_out[n_loads][4] = (block, occupied index,
+ * slot, last block that used the slot or -1) -- n_loads from tc_plan_summary, TC_ERR_WORKSPACE_TOO_SMALL if
+ * loads_capacity is less. */
+tc_status tc_plan_dump(int o, long long first, long long count, int nslots,
+                       int* recs_out, int* loads_out, long long loads_capacity);
 
 /* ---- a2: integral staging from DF factors --------------------------------------- */
 
@@ -130,6 +159,21 @@ tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v,
                                   void* stream, long long first, long long count,
                                   double* S_dev, double* E_partial_out);
 
+/* Host-resident amplitudes (the paper streams t2 pieces with cudaMemcpyAsync under the integral
+ * build, Fig. 2 l.6, 9: at o=150, v=1150 the amplitudes are 238 GB).  As
+ * tc_triples_energy_slice with DF input, except that `t2_host` is HOST memory (pinned for the copies to
+ * overlap; pageable works but serialises) and is never resident as a whole: the rows t2[x][:][:][:] that
+ * a block of triplets needs are copied into a device ring of slots on the library's side stream while the
+ * previous block computes, next to the slice cache.  eps, t1, DF factors: device.  Workspace size:
+ * tc_workspace_bytes_streamed. */
+tc_status tc_triples_energy_streamed(tc_ctx* ctx, int o, int v,
+                                     const double* eps_occ, const double* eps_vir,
+                                     const double* t1, const double* t2_host,
+                                     const tc_df_factors* df,
+                                     void* workspace, size_t workspace_bytes,
+                                     void* stream, long long first, long long count,
+                                     double* S_dev, double* E_partial_out);
+
 /* End-to-end variant with HOST inputs: copies the DF factors, amplitudes and orbital
  * energies to the device, assembles the integrals, computes E(T) over triplets
  * first .. first+count-1, returns it on the host.  This is the one call that allocates
@@ -145,10 +189,18 @@ tc_status tc_triples_energy_host(tc_ctx* ctx, int o, int v, int naux,
 
 /* Debug/validation: W_ijk^abc (eqs. (2),(5)) of one triplet written to W_dev[a][b][c]
  * (device, v^3) by the same tile kernels that feed the fused epilogue.  Any order of
- * i,j,k is accepted.  Used by the parity tests only. */
+ * i,j,k is accepted.  Used by the parity tests only (allocates its own scratch). */
 tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j, int k,
                              const double* t2, const tc_int_blocks* blocks,
                              double* W_dev, void* stream);
+/* Debug/validation: which W-builder kernel the next calls on ctx use.  TC_KERNEL_AUTO (default): the
+ * TMA/mbarrier kernel whenever the operands can be addressed by TMA (always, except for caller pointers
+ * that are not 16-byte aligned), else the cp.async kernel.  TC_KERNEL_CPASYNC forces the latter so the
+ * tests can check it on any input. */
+#define TC_KERNEL_AUTO    0
+#define TC_KERNEL_TMA     1
+#define TC_KERNEL_CPASYNC 2
+tc_status tc_debug_force_kernel(tc_ctx* ctx, int which);
 
 /* ---- statistics of the last energy call ----------------------------------------- */
 
@@ -161,6 +213,15 @@ typedef struct {
     double    ms_contraction;    /* device time of the fused W-builder kernels           */
     double    ms_staging;        /* device time of DF->block assembly (0 with blocks)    */
     long long slices_built;      /* (vv|v.) slices assembled from DF during the call     */
+    int       kernel;            /* W-builder that ran: TC_KERNEL_TMA or TC_KERNEL_CPASYNC */
+    int       padded;            /* 1: odd v, operands used through zero-padded copies (row length v+1) */
+    long long n_blocks;          /* blocked schedule: W-builder launches (0 = everything resident) */
+    long long t2_rows_copied;    /* streamed call: amplitude rows copied host->device    */
+    double    bytes_h2d;         /* streamed call: bytes copied host->device             */
+    double    ms_kernels;        /* sum of the W-builder launches alone (events around each launch)         */
+    double    ms_staging_side;   /* blocked schedule: device time of the side-stream staging (sum of spans)  */
+    double    staging_first_ms, staging_last_ms;          /* side-stream staging interval, relative to call start */
+    double    contraction_first_ms, contraction_last_ms;  /* first W-builder start / last W-builder end          */
 } tc_stats;
 tc_status tc_get_stats(const tc_ctx* ctx, tc_stats* out);
 
@@ -175,6 +236,13 @@ tc_status tc_bench_dfma_peak(tc_ctx* ctx, double seconds, double* tflops_sustain
 /* Device copy bandwidth (read+write bytes / time), GB/s, over `bytes` per direction
  * of caller-provided device buffers. */
 tc_status tc_bench_copy_bw(tc_ctx* ctx, void* dst_dev, const void* src_dev, size_t bytes, int reps, double* gbs);
+/* What the W-builder's consumer loop can reach: stand-alone kernels with the production kernel's warp
+ * tile (8 warps x 32 x 32, K chunk 4: 8 LDS.64 + 16 DMMA.8x8x4 per chunk), no flush, no epilogue.
+ *   variant 0: fragments from shared memory, no synchronisation      (the LDS + DMMA floor)
+ *   variant 1: + the 3-stage full/empty mbarrier ring, producers only arrive
+ *   variant 2: + real TMA producers streaming a device buffer (the production operand path)
+ * Returns TFLOP/s over about `seconds`.  `scratch_dev` (>= 64 MB, device) is the buffer variant 2 streams. */
+tc_status tc_bench_ring_peak(tc_ctx* ctx, int variant, double seconds, void* scratch_dev, size_t scratch_bytes, double* tflops);
 
 #ifdef __cplusplus
 }

@@ -158,3 +158,4 @@ def build_ovov(o, v, naux, Bov):
     out = np.empty((o, o, v, v), dtype=np.float64)
     lib().tco_build_ovov(o, v, naux, p, out.ctypes.data_as(_dp))
     return out
+from . import blocks  # noqa: E402,F401  (numpy statement of eq. (6), pinned against the C loops)

@@ -18,6 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtc_triples.so")
 
 TC_OK = 0
+TC_KERNEL_AUTO, TC_KERNEL_TMA, TC_KERNEL_CPASYNC = 0, 1, 2
 _STATUS = {0: "TC_OK", 1: "TC_ERR_INVALID_ARG", 2: "TC_ERR_UNSUPPORTED_DEVICE", 3: "TC_ERR_WORKSPACE_TOO_SMALL",
            4: "TC_ERR_CUDA", 5: "TC_ERR_INTERNAL"}
 
@@ -40,7 +41,11 @@ class TcStats(ctypes.Structure):
     _fields_ = [("n_triplets", ctypes.c_longlong), ("n_work_units", ctypes.c_longlong),
                 ("n_kernel_launches", ctypes.c_longlong), ("flop_contraction", ctypes.c_double),
                 ("ms_total", ctypes.c_double), ("ms_contraction", ctypes.c_double), ("ms_staging", ctypes.c_double),
-                ("slices_built", ctypes.c_longlong)]
+                ("slices_built", ctypes.c_longlong), ("kernel", ctypes.c_int), ("padded", ctypes.c_int),
+                ("n_blocks", ctypes.c_longlong), ("t2_rows_copied", ctypes.c_longlong), ("bytes_h2d", ctypes.c_double),
+                ("ms_kernels", ctypes.c_double), ("ms_staging_side", ctypes.c_double),
+                ("staging_first_ms", ctypes.c_double), ("staging_last_ms", ctypes.c_double),
+                ("contraction_first_ms", ctypes.c_double), ("contraction_last_ms", ctypes.c_double)]
 
     def as_dict(self):
         return {name: getattr(self, name) for name, _ in self._fields_}
@@ -48,10 +53,11 @@ class TcStats(ctypes.Structure):
 
 EXPORTS = [
     "tc_create", "tc_destroy", "tc_status_string", "tc_last_error",
-    "tc_triplet_count", "tc_triplet_decode", "tc_triplet_index",
-    "tc_workspace_bytes", "tc_build_blocks",
-    "tc_triples_energy", "tc_triples_energy_slice", "tc_triples_energy_host", "tc_debug_W_triplet",
-    "tc_get_stats", "tc_bench_dmma_peak", "tc_bench_dfma_peak", "tc_bench_copy_bw",
+    "tc_triplet_count", "tc_triplet_decode", "tc_triplet_index", "tc_triplet_partition",
+    "tc_workspace_bytes", "tc_workspace_bytes_streamed", "tc_plan_summary", "tc_plan_dump", "tc_build_blocks",
+    "tc_triples_energy", "tc_triples_energy_slice", "tc_triples_energy_streamed", "tc_triples_energy_host",
+    "tc_debug_W_triplet", "tc_debug_force_kernel",
+    "tc_get_stats", "tc_bench_dmma_peak", "tc_bench_dfma_peak", "tc_bench_copy_bw", "tc_bench_ring_peak",
 ]
 
 _lib = None
@@ -79,7 +85,14 @@ def lib() -> ctypes.CDLL:
     L.tc_triplet_decode.argtypes = [_i, _ll, _P(_i), _P(_i), _P(_i), _P(_d)]
     L.tc_triplet_index.argtypes = [_i, _i, _i, _i]
     L.tc_triplet_index.restype = _ll
+    L.tc_triplet_partition.argtypes = [_i, _i, _i, _P(_ll), _P(_ll)]
     L.tc_workspace_bytes.argtypes = [_vp, _i, _i, _i, _sz, _P(_sz)]
+    L.tc_workspace_bytes_streamed.argtypes = [_vp, _i, _i, _i, _sz, _P(_sz)]
+    L.tc_plan_summary.argtypes = [_i, _ll, _ll, _i, _P(_ll), _P(_ll), _P(_i), _P(_i), _P(_i)]
+    L.tc_plan_dump.argtypes = [_i, _ll, _ll, _i, _vp, _vp, _ll]
+    L.tc_triples_energy_streamed.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_DfFactors), _vp, _sz, _vp, _ll, _ll, _vp, _P(_d)]
+    L.tc_debug_force_kernel.argtypes = [_vp, _i]
+    L.tc_bench_ring_peak.argtypes = [_vp, _i, _d, _vp, _sz, _P(_d)]
     L.tc_build_blocks.argtypes = [_vp, _i, _i, _P(_DfFactors), _i, _i, _vp, _vp, _vp, _vp]
     L.tc_triples_energy.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_IntBlocks), _P(_DfFactors), _vp, _sz, _vp, _P(_d)]
     L.tc_triples_energy_slice.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_IntBlocks), _P(_DfFactors), _vp, _sz, _vp,
@@ -146,6 +159,11 @@ class Context:
         self._check(lib().tc_workspace_bytes(self._h, o, v, naux_or_0, hbm_budget, ctypes.byref(out)))
         return int(out.value)
 
+    def workspace_bytes_streamed(self, o: int, v: int, naux: int, hbm_budget: int = 0) -> int:
+        out = _sz()
+        self._check(lib().tc_workspace_bytes_streamed(self._h, o, v, naux, hbm_budget, ctypes.byref(out)))
+        return int(out.value)
+
     # -- a2 ----------------------------------------------------------------------------------
     def build_blocks(self, o, v, naux, Boo, Bov, Bvv, x0=0, nx=None, vvvo_out=None, ovoo_out=None, ovov_out=None,
                      stream=None):
@@ -164,8 +182,8 @@ class Context:
             d = _DfFactors(int(df[0]), _ptr(df[1]), _ptr(df[2]), _ptr(df[3]))
         return b, d, (ctypes.byref(b) if b is not None else None), (ctypes.byref(d) if d is not None else None)
 
-    def triples_energy(self, o, v, eps_occ, eps_vir, t1, t2, blocks=None, df=None, workspace=None,
-                       workspace_bytes=0, stream=None) -> float:
+    def triples_energy(self, o, v, eps_occ, eps_vir, t1, t2, *, workspace, workspace_bytes, blocks=None, df=None,
+                       stream=None) -> float:
         """blocks = (vvvo, ovoo, ovov) or df = (naux, Boo, Bov, Bvv); all device arrays."""
         b, d, pb, pd = self._ints(blocks, df)
         E = _d()
@@ -173,13 +191,24 @@ class Context:
                                             _ptr(workspace), workspace_bytes, _stream(stream), ctypes.byref(E)))
         return E.value
 
-    def triples_energy_slice(self, o, v, eps_occ, eps_vir, t1, t2, blocks=None, df=None, workspace=None,
-                             workspace_bytes=0, stream=None, first=0, count=0, S_dev=None) -> float:
+    def triples_energy_slice(self, o, v, eps_occ, eps_vir, t1, t2, *, workspace, workspace_bytes, blocks=None, df=None,
+                             stream=None, first=0, count=0, S_dev=None) -> float:
         b, d, pb, pd = self._ints(blocks, df)
         E = _d()
         self._check(lib().tc_triples_energy_slice(self._h, o, v, _ptr(eps_occ), _ptr(eps_vir), _ptr(t1), _ptr(t2), pb, pd,
                                                   _ptr(workspace), workspace_bytes, _stream(stream), first, count,
                                                   _ptr(S_dev), ctypes.byref(E)))
+        return E.value
+
+    def triples_energy_streamed(self, o, v, eps_occ, eps_vir, t1, t2_host, *, df, workspace, workspace_bytes, stream=None,
+                                first=0, count=0, S_dev=None) -> float:
+        """t2_host: C-contiguous float64 HOST array (numpy, or a pinned torch CPU tensor); everything else on the device."""
+        d = _DfFactors(int(df[0]), _ptr(df[1]), _ptr(df[2]), _ptr(df[3]))
+        t2p = t2_host.ctypes.data if isinstance(t2_host, np.ndarray) else _ptr(t2_host)
+        E = _d()
+        self._check(lib().tc_triples_energy_streamed(self._h, o, v, _ptr(eps_occ), _ptr(eps_vir), _ptr(t1), t2p, ctypes.byref(d),
+                                                     _ptr(workspace), workspace_bytes, _stream(stream), first, count,
+                                                     _ptr(S_dev), ctypes.byref(E)))
         return E.value
 
     def triples_energy_host(self, o, v, naux, eps_occ, eps_vir, t1, t2, Boo, Bov, Bvv, first=0, count=None):
@@ -195,6 +224,9 @@ class Context:
     def debug_W_triplet(self, o, v, i, j, k, t2, blocks: Sequence, W_dev, stream=None):
         b = _IntBlocks(*[_ptr(x) for x in blocks])
         self._check(lib().tc_debug_W_triplet(self._h, o, v, i, j, k, _ptr(t2), ctypes.byref(b), _ptr(W_dev), _stream(stream)))
+
+    def force_kernel(self, which: int = TC_KERNEL_AUTO):
+        self._check(lib().tc_debug_force_kernel(self._h, which))
 
     def get_stats(self) -> dict:
         s = TcStats()
@@ -216,6 +248,42 @@ class Context:
         g = _d()
         self._check(lib().tc_bench_copy_bw(self._h, _ptr(dst), _ptr(src), nbytes, reps, ctypes.byref(g)))
         return g.value
+
+
+    def bench_ring_peak(self, variant: int, seconds: float = 1.0, scratch=None, scratch_bytes: int = 0) -> float:
+        g = _d()
+        self._check(lib().tc_bench_ring_peak(self._h, variant, seconds, _ptr(scratch), scratch_bytes, ctypes.byref(g)))
+        return g.value
+
+
+def triplet_partition(o: int, world: int, rank: int):
+    """(first, count) of the linear triplet index owned by `rank` of `world` (host only)."""
+    f, c = _ll(), _ll()
+    rc = lib().tc_triplet_partition(o, world, rank, ctypes.byref(f), ctypes.byref(c))
+    if rc != TC_OK:
+        raise TcError(rc, "bad partition arguments")
+    return int(f.value), int(c.value)
+
+
+def plan_summary(o: int, first: int, count: int, nslots: int) -> dict:
+    """The blocked schedule for a triplet range with `nslots` operand slots (host only)."""
+    nb, nl, bi, bj, bk = _ll(), _ll(), _i(), _i(), _i()
+    rc = lib().tc_plan_summary(o, first, count, nslots, ctypes.byref(nb), ctypes.byref(nl), ctypes.byref(bi), ctypes.byref(bj),
+                               ctypes.byref(bk))
+    if rc != TC_OK:
+        raise TcError(rc, "no plan (bad range, or fewer than three slots)")
+    return {"n_blocks": int(nb.value), "n_loads": int(nl.value), "bi": bi.value, "bj": bj.value, "bk": bk.value}
+
+
+def plan_dump(o: int, first: int, count: int, nslots: int):
+    """(recs[count][8], loads[n_loads][4]) of the blocked schedule; see tc_plan_dump in the header."""
+    n_loads = plan_summary(o, first, count, nslots)["n_loads"]
+    recs = np.zeros((max(count, 1), 8), dtype=np.int32)
+    loads = np.zeros((max(n_loads, 1), 4), dtype=np.int32)
+    rc = lib().tc_plan_dump(o, first, count, nslots, recs.ctypes.data, loads.ctypes.data, n_loads)
+    if rc != TC_OK:
+        raise TcError(rc, "tc_plan_dump failed")
+    return recs[:count], loads[:n_loads]
 
 
 def triplet_count(o: int) -> int:

@@ -10,18 +10,30 @@
 
 #include "../../include/tc_triples.h"
 
+constexpr int TC_EV_RING = 16;     // fork/join events of the staging pipeline (blocked schedule)
+constexpr int TC_TIMING_RING = 64;  // timing-event pairs harvested as they are recycled
+
 struct tc_ctx {
     int device;
     int sm_count;
     int cc_major, cc_minor;
     size_t smem_optin;
     size_t l2_bytes;
-    cudaStream_t side_stream;      // integral staging runs here (a2)
-    cudaEvent_t ev_fork, ev_join;  // fork/join of side_stream against the caller's stream
+    // a2 on a side stream (blocked schedule): the slices / amplitude rows of block n+1 are staged here while the
+    // W-builder of block n runs on the caller's stream
+    cudaStream_t side_stream;
+    cudaEvent_t ev_fork;                    // caller's stream -> side stream at the start of a call
+    cudaEvent_t ev_staged[TC_EV_RING];      // side -> main: the operands of block n are in place
+    cudaEvent_t ev_done[TC_EV_RING];        // main -> side: the W-builder of block n has finished (its slots may be reused)
+    cudaEvent_t ev_k0[TC_TIMING_RING], ev_k1[TC_TIMING_RING];   // W-builder launch brackets (main stream)
+    cudaEvent_t ev_g0[TC_TIMING_RING], ev_g1[TC_TIMING_RING];   // staging brackets (side stream)
     cudaEvent_t ev_t0, ev_t1, ev_s0, ev_s1, ev_c0, ev_c1;
     double* pinned;                // a few doubles of pinned host memory for scalar results
     void* host_slab;               // device slab of tc_triples_energy_host, kept between calls (grow-only)
     size_t host_slab_bytes;
+    void* plan_host;               // pinned host staging of the blocked schedule's tables (grow-only)
+    size_t plan_host_bytes;
+    int force_kernel;              // tc_debug_force_kernel: 0 auto, 2 cp.async kernel (validation of the fallback)
     tc_stats stats;
     char err[512];
 };
@@ -78,19 +90,33 @@ cudaError_t tc_launch_df_gemm(const double* A, size_t lda, const double* B, size
                               int R2, long long sr1, long long sr2, int C2, long long sc1, long long sc2,
                               double* C, cudaStream_t stream);
 
-// a3-a6: fused W-builder + epilogue over a range of triplets (tc_wbuild.cu).
+// a3-a6: fused W-builder + epilogue over a list of triplets (tc_wbuild_tma.cu, tc_wbuild.cu).
+// One record per triplet.  The slots say where the per-occupied-index operands of the triplet live: slice slot s[p]
+// holds the (vv|v.) slice of occ[p], amplitude slot t[p] holds the row t2[occ[p]][:][:][:] (slot = index when
+// everything is resident; the blocked schedule and the host-resident t2 path cache them in fewer slots).
+struct tc_trip_rec {
+    int occ[3];   // i >= j >= k (tc_debug_W_triplet: any order)
+    int row;      // row of partial[]
+    int s[3];     // slice slots of i, j, k
+    int pad0;
+    int t[3];     // amplitude-row slots of i, j, k
+    int pad1;
+};
+static_assert(sizeof(tc_trip_rec) == 48, "tc_trip_rec is read as three int4");
+
 struct tc_wbuild_args {
     int o, v;
+    int ldv;                         // row length (doubles) of t2, ovoo and the slices: v, or v + 1 for odd v (padded copies)
     const double* eps_occ;
     const double* eps_vir;
     const double* t1;
-    const double* t2;
-    const double* const* slice_ptr;  // device array [o]: slice_ptr[x] -> I_x[d][b][c] (NULL if not resident)
-    bool slices_aligned16;           // every resident slice starts on a 16-byte boundary
-    const int* slice_slot;           // device array [o]: slot of slice x in the slice array the TMA map covers
-    const double* ovoo;
-    const double* ovov;
-    const int4* triplets;            // device array [n_trip]: (i, j, k, row of partial[])
+    const double* t2;                // [tslot][y][a][ldv], amplitude rows t2_row_stride doubles apart
+    size_t t2_row_stride;
+    const double* slices;            // slot s at slices + s * slice_stride, laid out [d][b][ldv]
+    size_t slice_stride;             // doubles
+    const double* ovoo;              // [z][x][l][ldv]
+    const double* ovov;              // [j][k][b][c] (unpadded; read by the epilogue only)
+    const tc_trip_rec* recs;         // device array [n_trip]
     int n_trip;
     double* partial;                 // device [n_trip][n_orbits] per-unit partial sums
     int n_orbits;
@@ -99,24 +125,32 @@ struct tc_wbuild_args {
 // TMA descriptors of the four operand streams of the main-path kernel (tc_wbuild_tma.cu).
 struct tc_wbuild_maps {
     CUtensorMap I;     // (vv|v.) slices   [slot][d][b][c]
-    CUtensorMap T2h;   // t2 as hole B     [y][l][n1][n2]
-    CUtensorMap T2p;   // t2 as particle A [x][y][m][d]
+    CUtensorMap T2h;   // t2 as hole B     [tslot][l][n1][n2]
+    CUtensorMap T2p;   // t2 as particle A [tslot][y][m][d]
     CUtensorMap Ovoo;  // (ov|oo) hole A   [z][x][l][m]
-    bool valid;        // false: v odd or a base pointer not 16-byte aligned -> cp.async fallback kernel
+    bool valid;        // false: a base pointer or stride is not 16-byte aligned -> cp.async fallback kernel
 };
-// slices: nslots slices of v^3 doubles, slice_stride doubles apart, starting at slice_base.
-cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, const double* slice_base, size_t slice_stride, int nslots,
-                                tc_wbuild_maps* out);
+// nslots slices and n_tslots amplitude rows behind a.slices / a.t2.
+cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, int nslots, int n_tslots, tc_wbuild_maps* out);
 int tc_wbuild_tile();                                  // virtual tile edge T
 int tc_wbuild_num_orbits(int v);                       // nb(nb+1)(nb+2)/6
-// maps == NULL or !maps->valid: cp.async kernel (any v); else the TMA/mbarrier kernel.
+// maps == NULL or !maps->valid: cp.async kernel (any alignment); else the TMA/mbarrier kernel.  Returns which ran
+// through *kernel_out (TC_KERNEL_TMA / TC_KERNEL_CPASYNC).
 cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const tc_wbuild_maps* maps,
-                             const int4* orbits /*device [n_orbits]: (A,B,C,0), A>=B>=C*/, cudaStream_t stream);
+                             const int4* orbits /*device [n_orbits]: (A,B,C,0), A>=B>=C*/, cudaStream_t stream, int* kernel_out);
 cudaError_t tc_launch_wbuild_cpasync(const tc_wbuild_args& a, const int4* orbits, cudaStream_t stream);
+// per-device kernel attributes (opt-in shared memory); called by tc_create with the device current
+cudaError_t tc_wbuild_configure();
+cudaError_t tc_wbuild_cpasync_configure();
+cudaError_t tc_stager_configure();
+cudaError_t tc_microbench_configure();
+
+// dst[r][0..v) = src[r][0..v), dst rows ldd doubles apart (ldd >= v; the pad is zeroed): TMA needs 16-byte row strides
+cudaError_t tc_launch_pad_rows(double* dst, size_t ldd, const double* src, size_t lds, size_t nrows, int v, cudaStream_t stream);
 
 // a7: deterministic reductions (tc_reduce.cu).
-//   triplets[t] = decode(first + t) as (i, j, k, t); w[t] = 2 - d_ij - d_jk
-cudaError_t tc_launch_make_triplets(int o, long long first, int n, int4* triplets, double* w, cudaStream_t stream);
+//   recs[t] = decode(first + t) with row = t and slots = indices; w[t] = 2 - d_ij - d_jk
+cudaError_t tc_launch_make_triplets(int o, long long first, int n, tc_trip_rec* recs, double* w, cudaStream_t stream);
 //   S[dest ? dest[t] : t] = sum_u partial[t][u], fixed order
 cudaError_t tc_launch_reduce_units(const double* partial, int n_trip, int n_units, const int* dest, double* S, cudaStream_t stream);
 //   *E = sum_t w[t] * S[t], fixed order, one block

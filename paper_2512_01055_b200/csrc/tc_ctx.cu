@@ -40,10 +40,20 @@ extern "C" tc_status tc_create(tc_ctx** out, int device) {
     bool ok = cudaSetDevice(device) == cudaSuccess;
     ok = ok && cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
-    ok = ok && cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) == cudaSuccess;
+    for (int n = 0; n < TC_EV_RING; n++) {
+        ok = ok && cudaEventCreateWithFlags(&ctx->ev_staged[n], cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&ctx->ev_done[n], cudaEventDisableTiming) == cudaSuccess;
+    }
+    for (int n = 0; n < TC_TIMING_RING; n++) {
+        ok = ok && cudaEventCreate(&ctx->ev_k0[n]) == cudaSuccess && cudaEventCreate(&ctx->ev_k1[n]) == cudaSuccess;
+        ok = ok && cudaEventCreate(&ctx->ev_g0[n]) == cudaSuccess && cudaEventCreate(&ctx->ev_g1[n]) == cudaSuccess;
+    }
     cudaEvent_t* timed[6] = {&ctx->ev_t0, &ctx->ev_t1, &ctx->ev_s0, &ctx->ev_s1, &ctx->ev_c0, &ctx->ev_c1};
     for (int n = 0; n < 6; n++) ok = ok && cudaEventCreate(timed[n]) == cudaSuccess;
     ok = ok && cudaMallocHost(&ctx->pinned, 64 * sizeof(double)) == cudaSuccess;
+    // opt-in shared memory of the kernels: a per-device attribute, set here for this context's device
+    ok = ok && tc_wbuild_configure() == cudaSuccess && tc_wbuild_cpasync_configure() == cudaSuccess &&
+         tc_stager_configure() == cudaSuccess && tc_microbench_configure() == cudaSuccess;
     if (!ok) {
         tc_destroy(ctx);
         return TC_ERR_CUDA;
@@ -56,11 +66,20 @@ extern "C" tc_status tc_destroy(tc_ctx* ctx) {
     if (!ctx) return TC_ERR_INVALID_ARG;
     cudaSetDevice(ctx->device);
     if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
-    cudaEvent_t evs[8] = {ctx->ev_fork, ctx->ev_join, ctx->ev_t0, ctx->ev_t1,
-                          ctx->ev_s0,   ctx->ev_s1,   ctx->ev_c0, ctx->ev_c1};
-    for (int n = 0; n < 8; n++)
+    cudaEvent_t evs[7] = {ctx->ev_fork, ctx->ev_t0, ctx->ev_t1, ctx->ev_s0, ctx->ev_s1, ctx->ev_c0, ctx->ev_c1};
+    for (int n = 0; n < 7; n++)
         if (evs[n]) cudaEventDestroy(evs[n]);
+    for (int n = 0; n < TC_EV_RING; n++) {
+        if (ctx->ev_staged[n]) cudaEventDestroy(ctx->ev_staged[n]);
+        if (ctx->ev_done[n]) cudaEventDestroy(ctx->ev_done[n]);
+    }
+    for (int n = 0; n < TC_TIMING_RING; n++) {
+        cudaEvent_t t4[4] = {ctx->ev_k0[n], ctx->ev_k1[n], ctx->ev_g0[n], ctx->ev_g1[n]};
+        for (int q = 0; q < 4; q++)
+            if (t4[q]) cudaEventDestroy(t4[q]);
+    }
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
+    if (ctx->plan_host) cudaFreeHost(ctx->plan_host);
     if (ctx->host_slab) cudaFree(ctx->host_slab);
     free(ctx);
     return TC_OK;

@@ -1,30 +1,42 @@
 // tc_energy.cu -- the C-ABI compute calls: argument checks, workspace carving, and the
 // launch sequence  scheduler (a1) -> stager (a2) -> fused W-builder/epilogue (a3-a6) -> reductions (a7).
-#include <stdlib.h>
-
+//
+// Two regimes.  RESIDENT: every (vv|v.) slice (and t2) is in HBM; one W-builder launch per batch of triplets, all on
+// the caller's stream.  BLOCKED (DF input whose slices do not fit, or host-resident t2): the per-occupied-index
+// operands are cached in slots, the triplets are executed block by block (tc_plan.cu), and the operands of block n+1
+// are staged on the library's side stream while the W-builder of block n runs on the caller's stream.
 #include <algorithm>
 #include <vector>
 
-#include "tc_common.cuh"
+#include "tc_plan.h"
 
 namespace {
 
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
+enum Mode { MODE_BLOCKS = 0, MODE_DF = 1, MODE_STREAMED = 2 };
+
 // How the caller's workspace is carved.  Everything the compute calls need lives here
 // (pre-allocate and reuse; no device allocation inside the call).
 struct Layout {
-    size_t off_orbits, off_sliceptr, off_sliceslot, off_trip, off_dest, off_w, off_S, off_partial, off_E, off_ovoo, off_ovov, off_vvvo;
+    size_t off_orbits, off_recs, off_dest, off_w, off_S, off_partial, off_E;
+    size_t off_t2;      // padded copy of t2 (odd v, resident t2) or the amplitude-row slots (streamed)
+    size_t off_ovoo;    // (ov|oo): assembled from DF, or the padded copy of the caller's block (odd v)
+    size_t off_ovov;    // (ov|ov) assembled from DF
+    size_t off_vvvo;    // slice slots: assembled from DF, or the padded copy of the caller's block (odd v)
     size_t total;
     int n_orbits;
-    int batch;      // triplets per W-builder launch
-    int n_slots;    // resident (vv|v.) slices (DF input): o = all materialised
+    int batch;          // triplets per W-builder launch (resident regime)
+    int n_slots;        // resident (vv|v.) slices; < o: blocked schedule
+    int ldv;            // row length of the TMA-addressed operands: v, or v + 1 when v is odd
+    size_t slice_stride, t2row_stride;   // doubles
 };
 
 constexpr size_t kPartialBudget = (size_t)256 << 20;
 
-bool make_layout(int o, int v, int naux, size_t budget, Layout* L) {
+// bounded == false: size for everything resident (tc_workspace_bytes with hbm_budget 0).
+bool make_layout(int o, int v, int naux, Mode mode, bool bounded, size_t budget, Layout* L) {
     const long long ntrip = (long long)o * (o + 1) * (o + 2) / 6;
     L->n_orbits = tc_wbuild_num_orbits(v);
     long long batch = (long long)(kPartialBudget / ((size_t)L->n_orbits * sizeof(double)));
@@ -32,6 +44,9 @@ bool make_layout(int o, int v, int naux, size_t budget, Layout* L) {
     if (batch > ntrip) batch = ntrip;
     if (batch * L->n_orbits > 0x7fffffffLL) batch = 0x7fffffffLL / L->n_orbits;
     L->batch = (int)batch;
+    L->ldv = v + (v & 1);
+    const bool pad = L->ldv != v;
+    const size_t O = o, V = v, LD = L->ldv;
     size_t off = 0;
     auto take = [&](size_t bytes) {
         size_t at = off;
@@ -39,34 +54,41 @@ bool make_layout(int o, int v, int naux, size_t budget, Layout* L) {
         return at;
     };
     L->off_orbits = take(sizeof(int4) * (size_t)L->n_orbits);
-    L->off_sliceptr = take(sizeof(double*) * (size_t)o);
-    L->off_sliceslot = take(sizeof(int) * (size_t)o);
-    L->off_trip = take(sizeof(int4) * (size_t)L->batch);
-    L->off_dest = take(sizeof(int) * (size_t)L->batch);
+    L->off_recs = take(sizeof(tc_trip_rec) * (size_t)ntrip);
+    L->off_dest = take(sizeof(int) * (size_t)ntrip);
     L->off_w = take(sizeof(double) * (size_t)ntrip);
     L->off_S = take(sizeof(double) * (size_t)ntrip);
     L->off_partial = take(sizeof(double) * (size_t)L->batch * L->n_orbits);
     L->off_E = take(sizeof(double) * 8);
-    L->off_ovoo = L->off_ovov = L->off_vvvo = 0;
-    L->n_slots = 0;
-    if (naux > 0) {
-        const size_t v3 = (size_t)v * v * v;
-        L->off_ovoo = take(sizeof(double) * (size_t)o * o * o * v);
-        L->off_ovov = take(sizeof(double) * (size_t)o * o * v * v);
-        const size_t slice_bytes = align_up(sizeof(double) * v3);
+    L->off_t2 = L->off_ovoo = L->off_ovov = L->off_vvvo = 0;
+    L->slice_stride = align_up(sizeof(double) * V * V * LD) / sizeof(double);
+    L->t2row_stride = align_up(sizeof(double) * O * V * LD) / sizeof(double);
+    L->n_slots = o;
+    if (mode == MODE_BLOCKS) {
+        if (pad) {   // TMA needs 16-byte row strides: zero-padded copies of the caller's arrays
+            L->off_t2 = take(sizeof(double) * O * L->t2row_stride);
+            L->off_ovoo = take(sizeof(double) * O * O * O * LD);
+            L->off_vvvo = take(sizeof(double) * O * L->slice_stride);
+        }
+    } else {
+        if (mode == MODE_DF && pad) L->off_t2 = take(sizeof(double) * O * L->t2row_stride);
+        L->off_ovoo = take(sizeof(double) * O * O * O * LD);
+        L->off_ovov = take(sizeof(double) * O * O * V * V);
+        const size_t per_slot = sizeof(double) * (L->slice_stride + (mode == MODE_STREAMED ? L->t2row_stride : 0));
         long long slots = o;
-        if (budget) {
+        if (bounded) {
             if (off >= budget) return false;
-            const long long fit = (long long)((budget - off) / slice_bytes);
+            const long long fit = (long long)((budget - off) / per_slot);
             if (fit < slots) slots = fit;
         }
-        // fewer slots than slices: the slice cache of the blocked schedule (needs i + one j + one k slice)
+        // fewer slots than slices: the blocked schedule (a triplet needs three operands resident)
         if (slots < 3 && slots < o) return false;
         L->n_slots = (int)slots;
-        L->off_vvvo = take(slice_bytes * (size_t)slots);
+        L->off_vvvo = take(sizeof(double) * L->slice_stride * (size_t)slots);
+        if (mode == MODE_STREAMED) L->off_t2 = take(sizeof(double) * L->t2row_stride * (size_t)slots);
     }
     L->total = off;
-    return budget == 0 || off <= budget;
+    return !bounded || off <= budget;
 }
 
 bool is_device_ptr(const void* p) {
@@ -80,12 +102,14 @@ bool is_device_ptr(const void* p) {
 }
 
 tc_status check_common(tc_ctx* ctx, int o, int v, const double* eps_occ, const double* eps_vir, const double* t1,
-                       const double* t2, const tc_int_blocks* blocks, const tc_df_factors* df) {
+                       const double* t2, bool t2_on_host, const tc_int_blocks* blocks, const tc_df_factors* df) {
     if (!ctx) return TC_ERR_INVALID_ARG;
     if (o < 1 || v < 1) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "o and v must be >= 1 (got o=%d v=%d)", o, v);
     if ((blocks != nullptr) == (df != nullptr)) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "exactly one of blocks / df must be given");
-    if (!is_device_ptr(eps_occ) || !is_device_ptr(eps_vir) || !is_device_ptr(t1) || !is_device_ptr(t2))
-        TC_FAIL(ctx, TC_ERR_INVALID_ARG, "eps_occ, eps_vir, t1, t2 must be device pointers");
+    if (!is_device_ptr(eps_occ) || !is_device_ptr(eps_vir) || !is_device_ptr(t1))
+        TC_FAIL(ctx, TC_ERR_INVALID_ARG, "eps_occ, eps_vir, t1 must be device pointers");
+    if (!t2_on_host && !is_device_ptr(t2)) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "t2 must be a device pointer");
+    if (t2_on_host && (!t2 || is_device_ptr(t2))) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "t2_host must be a host pointer");
     if (blocks && (!is_device_ptr(blocks->vvvo) || !is_device_ptr(blocks->ovoo) || !is_device_ptr(blocks->ovov)))
         TC_FAIL(ctx, TC_ERR_INVALID_ARG, "blocks->vvvo/ovoo/ovov must be device pointers");
     if (df && (df->naux < 1 || !is_device_ptr(df->Boo) || !is_device_ptr(df->Bov) || !is_device_ptr(df->Bvv)))
@@ -102,13 +126,343 @@ void fill_orbits(int v, std::vector<int4>& orb) {
             for (int C = 0; C <= B; C++) orb.push_back(make_int4(A, B, C, 0));
 }
 
+// ---- a2 launches: eq. (6) by the DMMA GEMM, outputs with row length ldv ----
+// slices x0 .. x0+nx-1 into dst (slice x at dst + (x - x0) * slice_stride, laid out [d][b][ldv])
+cudaError_t launch_slices(const tc_df_factors* df, int o, int v, int ldv, int x0, int nx, double* dst, size_t slice_stride,
+                          cudaStream_t st) {
+    // rows (d,b) -> d*v*ldv + b*ldv; cols (x,c) -> x*slice_stride + c
+    return tc_launch_df_gemm(df->Bvv, (size_t)v * v, df->Bov + (size_t)x0 * v, (size_t)o * v, v * v, nx * v, df->naux,
+                             /*R2*/ v, /*sr1*/ (long long)v * ldv, /*sr2*/ ldv, /*C2*/ v, /*sc1*/ (long long)slice_stride, /*sc2*/ 1, dst, st);
+}
+cudaError_t launch_ovoo(const tc_df_factors* df, int o, int v, int ldv, double* dst, cudaStream_t st) {
+    // ovoo[j][k][l][c]: rows (l,j) -> l*ldv + j*o*o*ldv; cols (k,c) -> k*o*ldv + c
+    const long long O = o, LD = ldv;
+    return tc_launch_df_gemm(df->Boo, (size_t)(O * O), df->Bov, (size_t)(O * v), o * o, o * v, df->naux,
+                             /*R2*/ o, /*sr1*/ LD, /*sr2*/ O * O * LD, /*C2*/ v, /*sc1*/ O * LD, /*sc2*/ 1, dst, st);
+}
+cudaError_t launch_ovov(const tc_df_factors* df, int o, int v, double* dst, cudaStream_t st) {
+    // ovov[j][k][b][c]: rows (j,b) -> j*o*v^2 + b*v; cols (k,c) -> k*v^2 + c
+    const long long O = o, V = v;
+    return tc_launch_df_gemm(df->Bov, (size_t)(O * V), df->Bov, (size_t)(O * V), o * v, o * v, df->naux,
+                             /*R2*/ v, /*sr1*/ O * V * V, /*sr2*/ V, /*C2*/ v, /*sc1*/ V * V, /*sc2*/ 1, dst, st);
+}
+
+// number of i=j=k triplets (weight 0) in [first, first+count): idx(i,i,i) = i(i+1)(i+2)/6 + i(i+1)/2 + i
+long long count_diagonal(int o, long long first, long long count) {
+    long long n = 0;
+    for (long long i = 0; i < o; i++) {
+        const long long idx = i * (i + 1) * (i + 2) / 6 + i * (i + 1) / 2 + i;
+        if (idx >= first && idx < first + count) n++;
+    }
+    return n;
+}
+
+struct TimingRing {
+    cudaEvent_t *e0, *e1;
+    long long used = 0;
+    double total_ms = 0;
+    TimingRing(cudaEvent_t* a, cudaEvent_t* b) : e0(a), e1(b) {}
+    void harvest(int slot) {
+        float ms = 0;
+        if (cudaEventSynchronize(e1[slot]) == cudaSuccess && cudaEventElapsedTime(&ms, e0[slot], e1[slot]) == cudaSuccess)
+            total_ms += ms;
+    }
+    int next() {
+        const int slot = (int)(used % TC_TIMING_RING);
+        if (used >= TC_TIMING_RING) harvest(slot);
+        used++;
+        return slot;
+    }
+    void finish() {
+        const long long n = std::min<long long>(used, TC_TIMING_RING);
+        const long long start = used - n;
+        for (long long q = start; q < used; q++) harvest((int)(q % TC_TIMING_RING));
+        used = 0;
+    }
+};
+
+// the energy call proper; t2 is a device pointer (MODE_BLOCKS / MODE_DF) or a host pointer (MODE_STREAMED)
+tc_status run_energy(tc_ctx* ctx, int o, int v, const double* eps_occ, const double* eps_vir, const double* t1,
+                     const double* t2, Mode mode, const tc_int_blocks* blocks, const tc_df_factors* df, void* workspace,
+                     size_t workspace_bytes, cudaStream_t s, long long first, long long count, double* S_dev,
+                     double* E_partial_out) {
+    const long long ntrip = tc_triplet_count(o);
+    if (first < 0 || count < 0 || first + count > ntrip)
+        TC_FAIL(ctx, TC_ERR_INVALID_ARG, "triplet range [%lld,%lld) outside [0,%lld)", first, first + count, ntrip);
+    if (!E_partial_out) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "E_out must not be NULL");
+    if (S_dev && !is_device_ptr(S_dev)) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "S_dev must be a device pointer");
+    Layout L;
+    // the caller's workspace_bytes is a hard bound: a layout that does not fit is an error, never an overrun
+    if (!is_device_ptr(workspace) || !make_layout(o, v, df ? df->naux : 0, mode, true, workspace_bytes, &L))
+        TC_FAIL(ctx, TC_ERR_WORKSPACE_TOO_SMALL, "workspace of %zu bytes is too small or not device memory (see tc_workspace_bytes)",
+                workspace_bytes);
+    TC_CUDA(ctx, cudaSetDevice(ctx->device));
+    char* ws = (char*)workspace;
+    int4* d_orbits = (int4*)(ws + L.off_orbits);
+    tc_trip_rec* d_recs = (tc_trip_rec*)(ws + L.off_recs);
+    int* d_dest = (int*)(ws + L.off_dest);
+    double* d_w = (double*)(ws + L.off_w);
+    double* d_S = (double*)(ws + L.off_S);
+    double* d_partial = (double*)(ws + L.off_partial);
+    double* d_E = (double*)(ws + L.off_E);
+    const int ldv = L.ldv;
+    const bool pad = ldv != v;
+    const size_t O = o, V = v;
+
+    memset(&ctx->stats, 0, sizeof(ctx->stats));
+    ctx->stats.padded = pad ? 1 : 0;
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_t0, s));
+
+    // ---- a2: integral staging, and the operand views the W-builder addresses ----
+    tc_wbuild_args a;
+    memset(&a, 0, sizeof(a));
+    a.o = o;
+    a.v = v;
+    a.eps_occ = eps_occ;
+    a.eps_vir = eps_vir;
+    a.t1 = t1;
+    a.n_orbits = L.n_orbits;
+    a.partial = d_partial;
+    a.recs = d_recs;
+    int n_tslots = o;
+    const bool blocked = (mode == MODE_STREAMED) || (mode == MODE_DF && L.n_slots < o);
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_s0, s));
+    if (mode == MODE_BLOCKS) {
+        a.ovov = blocks->ovov;
+        if (pad) {
+            double* p_t2 = (double*)(ws + L.off_t2);
+            double* p_ovoo = (double*)(ws + L.off_ovoo);
+            double* p_vvvo = (double*)(ws + L.off_vvvo);
+            for (int x = 0; x < o; x++) {
+                TC_CUDA(ctx, tc_launch_pad_rows(p_t2 + (size_t)x * L.t2row_stride, ldv, t2 + (size_t)x * O * V * V, V, O * V, v, s));
+                TC_CUDA(ctx, tc_launch_pad_rows(p_vvvo + (size_t)x * L.slice_stride, ldv, blocks->vvvo + (size_t)x * V * V * V, V, V * V, v, s));
+            }
+            TC_CUDA(ctx, tc_launch_pad_rows(p_ovoo, ldv, blocks->ovoo, V, O * O * O, v, s));
+            ctx->stats.n_kernel_launches += 2 * o + 1;
+            a.t2 = p_t2;
+            a.ovoo = p_ovoo;
+            a.slices = p_vvvo;
+            a.slice_stride = L.slice_stride;
+            a.ldv = ldv;
+        } else {
+            a.t2 = t2;
+            a.ovoo = blocks->ovoo;
+            a.slices = blocks->vvvo;
+            a.slice_stride = V * V * V;
+            a.ldv = v;
+        }
+    } else {
+        double* w_ovoo = (double*)(ws + L.off_ovoo);
+        double* w_ovov = (double*)(ws + L.off_ovov);
+        double* w_vvvo = (double*)(ws + L.off_vvvo);
+        TC_CUDA(ctx, launch_ovoo(df, o, v, ldv, w_ovoo, s));
+        TC_CUDA(ctx, launch_ovov(df, o, v, w_ovov, s));
+        ctx->stats.n_kernel_launches += 2;
+        if (!blocked) {
+            // all o slices in one launch
+            TC_CUDA(ctx, launch_slices(df, o, v, ldv, 0, o, w_vvvo, L.slice_stride, s));
+            ctx->stats.n_kernel_launches++;
+            ctx->stats.slices_built += o;
+        }
+        a.ovoo = w_ovoo;
+        a.ovov = w_ovov;
+        a.slices = w_vvvo;
+        a.slice_stride = L.slice_stride;
+        a.ldv = ldv;
+        if (mode == MODE_STREAMED) {
+            a.t2 = (double*)(ws + L.off_t2);   // amplitude-row slots [slot][y][a][ldv]
+            n_tslots = L.n_slots;
+        } else if (pad) {
+            double* p_t2 = (double*)(ws + L.off_t2);
+            for (int x = 0; x < o; x++)
+                TC_CUDA(ctx, tc_launch_pad_rows(p_t2 + (size_t)x * L.t2row_stride, ldv, t2 + (size_t)x * O * V * V, V, O * V, v, s));
+            ctx->stats.n_kernel_launches += o;
+            a.t2 = p_t2;
+        } else {
+            a.t2 = t2;
+        }
+    }
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_s1, s));
+    // amplitude rows: the caller's array has stride o*v*v, the padded copy / the slots sit at the aligned t2row_stride
+    a.t2_row_stride = (a.t2 == t2) ? O * V * V : L.t2row_stride;
+
+    // ---- tables: tile orbits (small host->device copy, stream ordered; the pageable source is staged before return) ----
+    {
+        std::vector<int4> orb;
+        fill_orbits(v, orb);
+        if ((int)orb.size() != L.n_orbits) TC_FAIL(ctx, TC_ERR_INTERNAL, "orbit count mismatch");
+        TC_CUDA(ctx, cudaMemcpyAsync(d_orbits, orb.data(), sizeof(int4) * orb.size(), cudaMemcpyHostToDevice, s));
+    }
+    tc_wbuild_maps maps;
+    TC_CUDA(ctx, tc_wbuild_make_maps(a, blocked ? L.n_slots : o, n_tslots, &maps));
+    if (ctx->force_kernel == TC_KERNEL_CPASYNC) maps.valid = false;
+    int kernel_ran = 0;
+
+    TimingRing kring(ctx->ev_k0, ctx->ev_k1), gring(ctx->ev_g0, ctx->ev_g1);
+    bool first_kernel = true, first_staging = true;
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_c0, s));
+    auto launch_block = [&](const tc_trip_rec* recs, int n, const int* dest, double* S_out) -> tc_status {
+        const int slot = kring.next();
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_k0[slot], s));
+        if (first_kernel) {
+            TC_CUDA(ctx, cudaEventRecord(ctx->ev_c0, s));
+            first_kernel = false;
+        }
+        a.recs = recs;
+        a.n_trip = n;
+        TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits, s, &kernel_ran));
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_k1[slot], s));
+        TC_CUDA(ctx, tc_launch_reduce_units(d_partial, n, L.n_orbits, dest, S_out, s));
+        ctx->stats.n_kernel_launches += 2;
+        ctx->stats.n_work_units += (long long)n * L.n_orbits;
+        return TC_OK;
+    };
+
+    if (!blocked) {
+        for (long long done = 0; done < count; done += L.batch) {
+            const int nb = (int)((count - done < L.batch) ? (count - done) : L.batch);
+            TC_CUDA(ctx, tc_launch_make_triplets(o, first + done, nb, d_recs, d_w + done, s));
+            ctx->stats.n_kernel_launches++;
+            tc_status st = launch_block(d_recs, nb, nullptr, d_S + done);
+            if (st != TC_OK) return st;
+        }
+    } else {
+        // ---- blocked schedule: tables uploaded once, then one W-builder launch per block with the next block's
+        //      operands staged on the side stream (a2 overlapped, north_star; PAPER.md:69 for the amplitudes) ----
+        tc_plan plan;
+        if (!tc_build_plan(o, first, count, L.n_slots, &plan)) TC_FAIL(ctx, TC_ERR_INTERNAL, "blocked schedule: no plan for %d slots", L.n_slots);
+        const size_t nrec = plan.recs.size();
+        if ((long long)nrec != count) TC_FAIL(ctx, TC_ERR_INTERNAL, "blocked schedule: %zu records for %lld triplets", nrec, count);
+        const size_t bytes_tab = nrec * (sizeof(tc_trip_rec) + sizeof(int) + sizeof(double)) + 64;
+        if (bytes_tab > ctx->plan_host_bytes) {
+            if (ctx->plan_host) cudaFreeHost(ctx->plan_host);
+            ctx->plan_host = nullptr;
+            ctx->plan_host_bytes = 0;
+            TC_CUDA(ctx, cudaMallocHost(&ctx->plan_host, bytes_tab));   // pinned HOST memory (grow-only); no device allocation
+            ctx->plan_host_bytes = bytes_tab;
+        }
+        if (nrec) {
+            tc_trip_rec* h_recs = (tc_trip_rec*)ctx->plan_host;
+            double* h_w = (double*)(h_recs + nrec);
+            int* h_dest = (int*)(h_w + nrec);
+            memcpy(h_recs, plan.recs.data(), nrec * sizeof(tc_trip_rec));
+            memcpy(h_dest, plan.dest.data(), nrec * sizeof(int));
+            for (size_t r = 0; r < nrec; r++) {   // w[dest] = 2 - d_ij - d_jk (eq. (1))
+                const tc_trip_rec& rec = plan.recs[r];
+                h_w[plan.dest[r]] = 2.0 - (rec.occ[0] == rec.occ[1] ? 1.0 : 0.0) - (rec.occ[1] == rec.occ[2] ? 1.0 : 0.0);
+            }
+            TC_CUDA(ctx, cudaMemcpyAsync(d_recs, h_recs, nrec * sizeof(tc_trip_rec), cudaMemcpyHostToDevice, s));
+            TC_CUDA(ctx, cudaMemcpyAsync(d_w, h_w, nrec * sizeof(double), cudaMemcpyHostToDevice, s));
+            TC_CUDA(ctx, cudaMemcpyAsync(d_dest, h_dest, nrec * sizeof(int), cudaMemcpyHostToDevice, s));
+        }
+        cudaStream_t side = ctx->side_stream;
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));         // the side stream starts after ovoo/ovov and the tables
+        TC_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
+        double* w_vvvo = (double*)(ws + L.off_vvvo);
+        double* w_t2 = (mode == MODE_STREAMED) ? (double*)(ws + L.off_t2) : nullptr;
+        const long long nblocks = (long long)plan.blocks.size();
+        for (long long n = 0; n < nblocks; n++) {
+            const tc_plan_block& b = plan.blocks[n];
+            if (b.load_end > b.load_begin) {
+                // the slots being overwritten were last read by block wait_block: wait for its W-builder.  The event ring
+                // holds the last TC_EV_RING blocks; an older block is covered by waiting for block n-2 (stream order).
+                long long wb = b.wait_block;
+                if (wb >= 0 && n - wb >= TC_EV_RING) wb = n - 2;
+                if (wb >= 0) TC_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_done[wb % TC_EV_RING], 0));
+                const int g = gring.next();
+                TC_CUDA(ctx, cudaEventRecord(ctx->ev_g0[g], side));
+                if (first_staging) {
+                    TC_CUDA(ctx, cudaEventRecord(ctx->ev_s0, side));
+                    first_staging = false;
+                }
+                for (int q = b.load_begin; q < b.load_end; q++) {
+                    const tc_plan_load& ld = plan.loads[q];
+                    TC_CUDA(ctx, launch_slices(df, o, v, ldv, ld.x, 1, w_vvvo + (size_t)ld.slot * L.slice_stride, L.slice_stride, side));
+                    ctx->stats.n_kernel_launches++;
+                    ctx->stats.slices_built++;
+                    if (w_t2) {   // the amplitude row t2[x][:][:][:] from the host, padded on the fly when v is odd
+                        TC_CUDA(ctx, cudaMemcpy2DAsync(w_t2 + (size_t)ld.slot * L.t2row_stride, sizeof(double) * ldv,
+                                                       t2 + (size_t)ld.x * O * V * V, sizeof(double) * V, sizeof(double) * V, O * V,
+                                                       cudaMemcpyHostToDevice, side));
+                        ctx->stats.t2_rows_copied++;
+                        ctx->stats.bytes_h2d += (double)(sizeof(double) * O * V * V);
+                    }
+                }
+                TC_CUDA(ctx, cudaEventRecord(ctx->ev_g1[g], side));
+                TC_CUDA(ctx, cudaEventRecord(ctx->ev_s1, side));
+                TC_CUDA(ctx, cudaEventRecord(ctx->ev_staged[n % TC_EV_RING], side));
+                TC_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_staged[n % TC_EV_RING], 0));
+            }
+            tc_status st = launch_block(d_recs + b.rec_begin, b.n, d_dest + b.rec_begin, d_S);
+            if (st != TC_OK) return st;
+            TC_CUDA(ctx, cudaEventRecord(ctx->ev_done[n % TC_EV_RING], s));
+        }
+        ctx->stats.n_blocks = nblocks;
+        // every ev_staged has been waited for on the caller's stream: the side stream is joined
+    }
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_c1, s));
+    TC_CUDA(ctx, tc_launch_reduce_energy(d_S, d_w, count, d_E, s));
+    ctx->stats.n_kernel_launches++;
+    if (S_dev && count > 0) TC_CUDA(ctx, cudaMemcpyAsync(S_dev, d_S, sizeof(double) * (size_t)count, cudaMemcpyDeviceToDevice, s));
+    TC_CUDA(ctx, cudaMemcpyAsync(ctx->pinned, d_E, sizeof(double), cudaMemcpyDeviceToHost, s));
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_t1, s));
+    TC_CUDA(ctx, cudaStreamSynchronize(s));
+    TC_CUDA(ctx, cudaStreamSynchronize(ctx->side_stream));
+
+    float ms = 0;
+    cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_t1);
+    ctx->stats.ms_total = ms;
+    if (count > 0) {
+        cudaEventElapsedTime(&ms, ctx->ev_c0, ctx->ev_c1);
+        ctx->stats.ms_contraction = ms;
+        cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_c0);
+        ctx->stats.contraction_first_ms = ms;
+        cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_c1);
+        ctx->stats.contraction_last_ms = ms;
+    }
+    kring.finish();
+    ctx->stats.ms_kernels = kring.total_ms;
+    if (!blocked) {
+        if (df) {
+            cudaEventElapsedTime(&ms, ctx->ev_s0, ctx->ev_s1);
+            ctx->stats.ms_staging = ms;
+        }
+    } else {
+        gring.finish();
+        ctx->stats.ms_staging_side = gring.total_ms;
+        ctx->stats.ms_staging = gring.total_ms;
+        if (!first_staging) {
+            cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_s0);
+            ctx->stats.staging_first_ms = ms;
+            cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_s1);
+            ctx->stats.staging_last_ms = ms;
+        }
+    }
+    ctx->stats.kernel = kernel_ran;
+    const long long nz = count - count_diagonal(o, first, count);
+    ctx->stats.n_triplets = nz;
+    ctx->stats.flop_contraction = (double)nz * 12.0 * (double)v * v * v * ((double)v + o);
+    *E_partial_out = (count > 0) ? ctx->pinned[0] : 0.0;
+    return TC_OK;
+}
+
 }  // namespace
 
 extern "C" tc_status tc_workspace_bytes(tc_ctx* ctx, int o, int v, int naux_or_0, size_t hbm_budget, size_t* bytes) {
     if (!ctx || !bytes) return TC_ERR_INVALID_ARG;
     if (o < 1 || v < 1 || naux_or_0 < 0) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "bad sizes o=%d v=%d naux=%d", o, v, naux_or_0);
     Layout L;
-    if (!make_layout(o, v, naux_or_0, hbm_budget, &L))
+    if (!make_layout(o, v, naux_or_0, naux_or_0 ? MODE_DF : MODE_BLOCKS, hbm_budget != 0, hbm_budget, &L))
+        TC_FAIL(ctx, TC_ERR_WORKSPACE_TOO_SMALL, "problem does not fit the HBM budget of %zu bytes", hbm_budget);
+    *bytes = L.total;
+    return TC_OK;
+}
+
+extern "C" tc_status tc_workspace_bytes_streamed(tc_ctx* ctx, int o, int v, int naux, size_t hbm_budget, size_t* bytes) {
+    if (!ctx || !bytes) return TC_ERR_INVALID_ARG;
+    if (o < 1 || v < 1 || naux < 1) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "bad sizes o=%d v=%d naux=%d", o, v, naux);
+    Layout L;
+    if (!make_layout(o, v, naux, MODE_STREAMED, hbm_budget != 0, hbm_budget, &L))
         TC_FAIL(ctx, TC_ERR_WORKSPACE_TOO_SMALL, "problem does not fit the HBM budget of %zu bytes", hbm_budget);
     *bytes = L.total;
     return TC_OK;
@@ -123,25 +477,17 @@ extern "C" tc_status tc_build_blocks(tc_ctx* ctx, int o, int v, const tc_df_fact
     if (vvvo_out && (x0 < 0 || nx < 0 || x0 + nx > o)) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "slice range [%d,%d) outside [0,%d)", x0, x0 + nx, o);
     TC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
-    const int naux = df->naux;
-    const long long V = v, O = o;
     if (vvvo_out && nx > 0) {
-        // rows (d,b) -> d*v + b (row*v), cols (x,c) -> x*v^3 + c
-        TC_CUDA(ctx, tc_launch_df_gemm(df->Bvv, (size_t)(V * V), df->Bov + (size_t)x0 * v, (size_t)(O * V), v * v, nx * v, naux,
-                                       /*R2*/ 1, /*sr1*/ V, /*sr2*/ 0, /*C2*/ v, /*sc1*/ V * V * V, /*sc2*/ 1, vvvo_out, st));
+        TC_CUDA(ctx, launch_slices(df, o, v, v, x0, nx, vvvo_out, (size_t)v * v * v, st));
         ctx->stats.n_kernel_launches++;
         ctx->stats.slices_built += nx;
     }
     if (ovoo_out) {
-        // rows (l,j): l*v + j*o^2*v; cols (k,c): k*o*v + c
-        TC_CUDA(ctx, tc_launch_df_gemm(df->Boo, (size_t)(O * O), df->Bov, (size_t)(O * V), o * o, o * v, naux,
-                                       /*R2*/ o, /*sr1*/ V, /*sr2*/ O * O * V, /*C2*/ v, /*sc1*/ O * V, /*sc2*/ 1, ovoo_out, st));
+        TC_CUDA(ctx, launch_ovoo(df, o, v, v, ovoo_out, st));
         ctx->stats.n_kernel_launches++;
     }
     if (ovov_out) {
-        // rows (j,b): j*o*v^2 + b*v; cols (k,c): k*v^2 + c
-        TC_CUDA(ctx, tc_launch_df_gemm(df->Bov, (size_t)(O * V), df->Bov, (size_t)(O * V), o * v, o * v, naux,
-                                       /*R2*/ v, /*sr1*/ O * V * V, /*sr2*/ V, /*C2*/ v, /*sc1*/ V * V, /*sc2*/ 1, ovov_out, st));
+        TC_CUDA(ctx, launch_ovov(df, o, v, ovov_out, st));
         ctx->stats.n_kernel_launches++;
     }
     return TC_OK;
@@ -151,244 +497,22 @@ extern "C" tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v, const do
                                              const double* t1, const double* t2, const tc_int_blocks* blocks,
                                              const tc_df_factors* df, void* workspace, size_t workspace_bytes, void* stream,
                                              long long first, long long count, double* S_dev, double* E_partial_out) {
-    tc_status st = check_common(ctx, o, v, eps_occ, eps_vir, t1, t2, blocks, df);
+    tc_status st = check_common(ctx, o, v, eps_occ, eps_vir, t1, t2, false, blocks, df);
     if (st != TC_OK) return st;
-    const long long ntrip = tc_triplet_count(o);
-    if (first < 0 || count < 0 || first + count > ntrip)
-        TC_FAIL(ctx, TC_ERR_INVALID_ARG, "triplet range [%lld,%lld) outside [0,%lld)", first, first + count, ntrip);
-    if (!E_partial_out) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "E_out must not be NULL");
-    if (S_dev && !is_device_ptr(S_dev)) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "S_dev must be a device pointer");
-    Layout L;
-    if (!make_layout(o, v, df ? df->naux : 0, workspace_bytes, &L) || !is_device_ptr(workspace))
-        TC_FAIL(ctx, TC_ERR_WORKSPACE_TOO_SMALL, "workspace of %zu bytes is too small or not device memory (see tc_workspace_bytes)",
-                workspace_bytes);
-    TC_CUDA(ctx, cudaSetDevice(ctx->device));
-    cudaStream_t s = (cudaStream_t)stream;
-    char* ws = (char*)workspace;
-    int4* d_orbits = (int4*)(ws + L.off_orbits);
-    const double** d_sliceptr = (const double**)(ws + L.off_sliceptr);
-    int* d_sliceslot = (int*)(ws + L.off_sliceslot);
-    int4* d_trip = (int4*)(ws + L.off_trip);
-    int* d_dest = (int*)(ws + L.off_dest);
-    double* d_w = (double*)(ws + L.off_w);
-    double* d_S = (double*)(ws + L.off_S);
-    double* d_partial = (double*)(ws + L.off_partial);
-    double* d_E = (double*)(ws + L.off_E);
+    return run_energy(ctx, o, v, eps_occ, eps_vir, t1, t2, df ? MODE_DF : MODE_BLOCKS, blocks, df, workspace, workspace_bytes,
+                      (cudaStream_t)stream, first, count, S_dev, E_partial_out);
+}
 
-    memset(&ctx->stats, 0, sizeof(ctx->stats));
-    TC_CUDA(ctx, cudaEventRecord(ctx->ev_t0, s));
-
-    // ---- a2: integral staging ----
-    const double *ovoo, *ovov, *vvvo;
-    size_t slice_stride;
-    if (df) {
-        double* w_ovoo = (double*)(ws + L.off_ovoo);
-        double* w_ovov = (double*)(ws + L.off_ovov);
-        double* w_vvvo = (double*)(ws + L.off_vvvo);
-        TC_CUDA(ctx, cudaEventRecord(ctx->ev_s0, s));
-        st = tc_build_blocks(ctx, o, v, df, 0, o, nullptr, w_ovoo, w_ovov, s);
-        if (st != TC_OK) return st;
-        // slices land at an aligned stride so each starts on a 256-byte boundary
-        slice_stride = align_up(sizeof(double) * (size_t)v * v * v) / sizeof(double);
-        if (L.n_slots >= o) {
-            // all o slices in one launch: column (x, c) of the v^2 x (o v) product lands at x * slice_stride + c
-            TC_CUDA(ctx, tc_launch_df_gemm(df->Bvv, (size_t)v * v, df->Bov, (size_t)o * v, v * v, o * v, df->naux, 1, (long long)v, 0,
-                                           v, (long long)slice_stride, 1, w_vvvo, s));
-            ctx->stats.n_kernel_launches++;
-            ctx->stats.slices_built += o;
-        }
-        TC_CUDA(ctx, cudaEventRecord(ctx->ev_s1, s));
-        ovoo = w_ovoo;
-        ovov = w_ovov;
-        vvvo = w_vvvo;
-    } else {
-        ovoo = blocks->ovoo;
-        ovov = blocks->ovov;
-        vvvo = blocks->vvvo;
-        slice_stride = (size_t)v * v * v;
-    }
-
-    // ---- tables: tile orbits and slice pointers (small host->device copies, stream ordered) ----
-    {
-        std::vector<int4> orb;
-        fill_orbits(v, orb);
-        if ((int)orb.size() != L.n_orbits) TC_FAIL(ctx, TC_ERR_INTERNAL, "orbit count mismatch");
-        std::vector<const double*> sp(o);
-        std::vector<int> slot(o);
-        for (int x = 0; x < o; x++) {
-            sp[x] = vvvo + (size_t)x * slice_stride;
-            slot[x] = x;  // all slices resident, slice x in slot x
-        }
-        TC_CUDA(ctx, cudaMemcpyAsync(d_sliceslot, slot.data(), sizeof(int) * slot.size(), cudaMemcpyHostToDevice, s));
-        // pageable sources: cudaMemcpyAsync stages them before returning, so the vectors may die here
-        TC_CUDA(ctx, cudaMemcpyAsync(d_orbits, orb.data(), sizeof(int4) * orb.size(), cudaMemcpyHostToDevice, s));
-        TC_CUDA(ctx, cudaMemcpyAsync(d_sliceptr, sp.data(), sizeof(double*) * sp.size(), cudaMemcpyHostToDevice, s));
-        TC_CUDA(ctx, cudaStreamSynchronize(s));
-    }
-
-    // ---- a1 + a3..a7 over batches of triplets ----
-    tc_wbuild_args a;
-    a.o = o;
-    a.v = v;
-    a.eps_occ = eps_occ;
-    a.eps_vir = eps_vir;
-    a.t1 = t1;
-    a.t2 = t2;
-    a.slice_ptr = d_sliceptr;
-    a.slices_aligned16 = ((uintptr_t)vvvo % 16 == 0) && ((slice_stride * sizeof(double)) % 16 == 0);
-    a.ovoo = ovoo;
-    a.ovov = ovov;
-    a.triplets = d_trip;
-    a.partial = d_partial;
-    a.n_orbits = L.n_orbits;
-    a.slice_slot = d_sliceslot;
-    a.W_debug = nullptr;
-    const bool blocked = df && L.n_slots < o;
-    const int nslots = blocked ? L.n_slots : o;
-    tc_wbuild_maps maps;
-    TC_CUDA(ctx, tc_wbuild_make_maps(a, vvvo, slice_stride, nslots, &maps));
-    if (getenv("TC_FORCE_CPASYNC")) maps.valid = false;  // testing aid: exercise the fallback kernel on even v
-    TC_CUDA(ctx, cudaEventRecord(ctx->ev_c0, s));
-    if (!blocked) {
-        for (long long done = 0; done < count; done += L.batch) {
-            const int nb = (int)((count - done < L.batch) ? (count - done) : L.batch);
-            TC_CUDA(ctx, tc_launch_make_triplets(o, first + done, nb, d_trip, d_w + done, s));
-            a.n_trip = nb;
-            TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits, s));
-            TC_CUDA(ctx, tc_launch_reduce_units(d_partial, nb, L.n_orbits, nullptr, d_S + done, s));
-            ctx->stats.n_kernel_launches += 3;
-            ctx->stats.n_work_units += (long long)nb * L.n_orbits;
-        }
-    } else {
-        // ---- blocked schedule with a slice cache ("LRU of slots" for cfg4-size problems) ----
-        // The (vv|v.) slices do not all fit: nslots slots hold the slices a block of triplets needs.  For each
-        // i the (j,k) plane is cut into b x b blocks, b = (nslots-1)/2: slice i stays pinned, a block of j slices
-        // stays while the k blocks stream through, so a block of up to b^2 triplets costs at most b new slices.
-        // Missing slices are assembled from the DF factors (eq. (6)) right before the launch that needs them.
-        for (long long done = 0; done < count; done += L.batch) {  // weights of the whole range
-            const int nb = (int)((count - done < L.batch) ? (count - done) : L.batch);
-            TC_CUDA(ctx, tc_launch_make_triplets(o, first + done, nb, d_trip, d_w + done, s));
-            ctx->stats.n_kernel_launches++;
-        }
-        double* w_vvvo = (double*)(ws + L.off_vvvo);
-        const int b = std::max(1, (nslots - 1) / 2);
-        std::vector<int> slot_of(o, -1), owner(nslots, -1);
-        std::vector<long long> stamp(nslots, 0);
-        long long tick = 0;
-        std::vector<const double*> sp(o, nullptr);
-        std::vector<int4> list;
-        std::vector<int> dest;
-        auto flush_list = [&]() -> tc_status {
-            for (size_t at = 0; at < list.size(); at += (size_t)L.batch) {
-                const int nb = (int)std::min((size_t)L.batch, list.size() - at);
-                for (int t = 0; t < nb; t++) list[at + t].w = t;
-                TC_CUDA(ctx, cudaMemcpyAsync(d_trip, list.data() + at, sizeof(int4) * nb, cudaMemcpyHostToDevice, s));
-                TC_CUDA(ctx, cudaMemcpyAsync(d_dest, dest.data() + at, sizeof(int) * nb, cudaMemcpyHostToDevice, s));
-                TC_CUDA(ctx, cudaMemcpyAsync(d_sliceslot, slot_of.data(), sizeof(int) * o, cudaMemcpyHostToDevice, s));
-                TC_CUDA(ctx, cudaMemcpyAsync(d_sliceptr, sp.data(), sizeof(double*) * o, cudaMemcpyHostToDevice, s));
-                a.n_trip = nb;
-                TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits, s));
-                TC_CUDA(ctx, tc_launch_reduce_units(d_partial, nb, L.n_orbits, d_dest, d_S, s));
-                ctx->stats.n_kernel_launches += 2;
-                ctx->stats.n_work_units += (long long)nb * L.n_orbits;
-            }
-            list.clear();
-            dest.clear();
-            return TC_OK;
-        };
-        // make slice x resident without evicting any slice of `keep`
-        auto ensure = [&](int x, const std::vector<int>& keep) -> tc_status {
-            if (slot_of[x] >= 0) {
-                stamp[slot_of[x]] = ++tick;
-                return TC_OK;
-            }
-            int victim = -1;
-            for (int q = 0; q < nslots; q++) {
-                if (owner[q] >= 0 && std::find(keep.begin(), keep.end(), owner[q]) != keep.end()) continue;
-                if (victim < 0 || owner[q] < 0 || (owner[victim] >= 0 && stamp[q] < stamp[victim])) victim = q;
-                if (owner[q] < 0) break;
-            }
-            if (victim < 0) TC_FAIL(ctx, TC_ERR_INTERNAL, "slice cache: no evictable slot");
-            if (owner[victim] >= 0) {
-                slot_of[owner[victim]] = -1;
-                sp[owner[victim]] = nullptr;
-            }
-            double* dst = w_vvvo + (size_t)victim * slice_stride;
-            TC_CUDA(ctx, tc_launch_df_gemm(df->Bvv, (size_t)v * v, df->Bov + (size_t)x * v, (size_t)o * v, v * v, v, df->naux, 1,
-                                           (long long)v, 0, v, 0, 1, dst, s));
-            ctx->stats.n_kernel_launches++;
-            ctx->stats.slices_built++;
-            owner[victim] = x;
-            slot_of[x] = victim;
-            sp[x] = dst;
-            stamp[victim] = ++tick;
-            return TC_OK;
-        };
-        long long idx = first;
-        const long long end = first + count;
-        while (idx < end) {
-            int i, j, k;
-            tc_triplet_decode(o, idx, &i, &j, &k, nullptr);
-            // the (j,k) pairs of this i inside the range: idx .. min(end, start of i+1)
-            const long long next_i = (long long)(i + 1) * (i + 2) * (i + 3) / 6;
-            const long long stop = std::min(end, next_i);
-            std::vector<int4> pairs;  // (j, k, dest, 0)
-            for (long long n = idx; n < stop; n++) {
-                int ii, jj, kk;
-                tc_triplet_decode(o, n, &ii, &jj, &kk, nullptr);
-                pairs.push_back(make_int4(jj, kk, (int)(n - first), 0));
-            }
-            const int jmin = pairs.front().x, jmax = pairs.back().x;
-            for (int j0 = (jmin / b) * b; j0 <= jmax; j0 += b) {
-                for (int k0 = 0; k0 <= std::min(j0 + b - 1, jmax); k0 += b) {
-                    std::vector<int> need(1, i);
-                    for (const int4& pr : pairs) {
-                        if (pr.x < j0 || pr.x >= j0 + b || pr.y < k0 || pr.y >= k0 + b) continue;
-                        list.push_back(make_int4(i, pr.x, pr.y, 0));
-                        dest.push_back(pr.z);
-                        if (std::find(need.begin(), need.end(), pr.x) == need.end()) need.push_back(pr.x);
-                        if (std::find(need.begin(), need.end(), pr.y) == need.end()) need.push_back(pr.y);
-                    }
-                    if (list.empty()) continue;
-                    for (int x : need) {
-                        st = ensure(x, need);
-                        if (st != TC_OK) return st;
-                    }
-                    st = flush_list();
-                    if (st != TC_OK) return st;
-                }
-            }
-            idx = stop;
-        }
-    }
-    TC_CUDA(ctx, cudaEventRecord(ctx->ev_c1, s));
-    TC_CUDA(ctx, tc_launch_reduce_energy(d_S, d_w, count, d_E, s));
-    ctx->stats.n_kernel_launches++;
-    if (S_dev && count > 0) TC_CUDA(ctx, cudaMemcpyAsync(S_dev, d_S, sizeof(double) * (size_t)count, cudaMemcpyDeviceToDevice, s));
-    TC_CUDA(ctx, cudaMemcpyAsync(ctx->pinned, d_E, sizeof(double), cudaMemcpyDeviceToHost, s));
-    TC_CUDA(ctx, cudaEventRecord(ctx->ev_t1, s));
-    TC_CUDA(ctx, cudaStreamSynchronize(s));
-
-    float ms = 0;
-    cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_t1);
-    ctx->stats.ms_total = ms;
-    cudaEventElapsedTime(&ms, ctx->ev_c0, ctx->ev_c1);
-    ctx->stats.ms_contraction = ms;
-    if (df) {
-        cudaEventElapsedTime(&ms, ctx->ev_s0, ctx->ev_s1);
-        ctx->stats.ms_staging = ms;
-    }
-    long long nz = 0;
-    for (long long n = 0; n < count; n++) {
-        int i, j, k;
-        double w;
-        tc_triplet_decode(o, first + n, &i, &j, &k, &w);
-        if (w != 0.0) nz++;
-    }
-    ctx->stats.n_triplets = nz;
-    ctx->stats.flop_contraction = (double)nz * 12.0 * (double)v * v * v * ((double)v + o);
-    *E_partial_out = (count > 0) ? ctx->pinned[0] : 0.0;
-    return TC_OK;
+extern "C" tc_status tc_triples_energy_streamed(tc_ctx* ctx, int o, int v, const double* eps_occ, const double* eps_vir,
+                                                const double* t1, const double* t2_host, const tc_df_factors* df,
+                                                void* workspace, size_t workspace_bytes, void* stream, long long first,
+                                                long long count, double* S_dev, double* E_partial_out) {
+    if (!ctx) return TC_ERR_INVALID_ARG;
+    if (!df) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "the streamed call takes DF factors");
+    tc_status st = check_common(ctx, o, v, eps_occ, eps_vir, t1, t2_host, true, nullptr, df);
+    if (st != TC_OK) return st;
+    return run_energy(ctx, o, v, eps_occ, eps_vir, t1, t2_host, MODE_STREAMED, nullptr, df, workspace, workspace_bytes,
+                      (cudaStream_t)stream, first, count, S_dev, E_partial_out);
 }
 
 extern "C" tc_status tc_triples_energy(tc_ctx* ctx, int o, int v, const double* eps_occ, const double* eps_vir,
@@ -449,6 +573,14 @@ extern "C" tc_status tc_triples_energy_host(tc_ctx* ctx, int o, int v, int naux,
     return st;
 }
 
+extern "C" tc_status tc_debug_force_kernel(tc_ctx* ctx, int which) {
+    if (!ctx) return TC_ERR_INVALID_ARG;
+    if (which != TC_KERNEL_AUTO && which != TC_KERNEL_TMA && which != TC_KERNEL_CPASYNC)
+        TC_FAIL(ctx, TC_ERR_INVALID_ARG, "unknown kernel selector %d", which);
+    ctx->force_kernel = which;
+    return TC_OK;
+}
+
 extern "C" tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j, int k, const double* t2,
                                         const tc_int_blocks* blocks, double* W_dev, void* stream) {
     if (!ctx) return TC_ERR_INVALID_ARG;
@@ -459,50 +591,70 @@ extern "C" tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j,
         TC_FAIL(ctx, TC_ERR_INVALID_ARG, "t2, blocks and W_dev must be device pointers");
     TC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t s = (cudaStream_t)stream;
+    Layout L;
+    make_layout(o, v, 0, MODE_BLOCKS, false, 0, &L);
+    // debug path: scratch allocated here (not a compute call of the hot path); zeros stand in for eps and t1
+    const size_t b_zero = align_up(sizeof(double) * (size_t)(o > v ? o : v) * v);
+    char* tmp = nullptr;
+    TC_CUDA(ctx, cudaMalloc(&tmp, L.total + b_zero));
+    const int ldv = L.ldv;
+    const bool pad = ldv != v;
+    const size_t O = o, V = v;
     std::vector<int4> orb;
     fill_orbits(v, orb);
-    std::vector<const double*> sp(o);
-    for (int x = 0; x < o; x++) sp[x] = blocks->vvvo + (size_t)x * v * v * v;
-    // debug path: small temporaries allocated here (not a compute call of the hot path)
-    char* tmp = nullptr;
-    const size_t b_orb = align_up(sizeof(int4) * orb.size()), b_sp = align_up(sizeof(double*) * o + sizeof(int) * o);
-    const size_t b_part = align_up(sizeof(double) * orb.size());
-    const size_t b_dummy = align_up(sizeof(double) * (size_t)(o > v ? o : v) * v);
-    TC_CUDA(ctx, cudaMalloc(&tmp, b_orb + b_sp + 256 + b_part + b_dummy));
-    int4 trip = make_int4(i, j, k, 0);
-    cudaError_t e = cudaMemcpyAsync(tmp, orb.data(), sizeof(int4) * orb.size(), cudaMemcpyHostToDevice, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(tmp + b_orb, sp.data(), sizeof(double*) * o, cudaMemcpyHostToDevice, s);
-    std::vector<int> slot(o);
-    for (int x = 0; x < o; x++) slot[x] = x;
-    if (e == cudaSuccess)
-        e = cudaMemcpyAsync(tmp + b_orb + sizeof(double*) * o, slot.data(), sizeof(int) * o, cudaMemcpyHostToDevice, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(tmp + b_orb + b_sp, &trip, sizeof(int4), cudaMemcpyHostToDevice, s);
-    if (e == cudaSuccess) e = cudaMemsetAsync(tmp + b_orb + b_sp + 256 + b_part, 0, b_dummy, s);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    if (e == cudaSuccess) {
-        tc_wbuild_args a;
-        a.o = o;
-        a.v = v;
-        const double* zeros = (const double*)(tmp + b_orb + b_sp + 256 + b_part);
-        a.eps_occ = zeros;  // the epilogue result is discarded; only W is wanted
-        a.eps_vir = zeros;
-        a.t1 = zeros;
+    tc_trip_rec rec;
+    memset(&rec, 0, sizeof(rec));
+    rec.occ[0] = i; rec.occ[1] = j; rec.occ[2] = k;
+    for (int p = 0; p < 3; p++) rec.s[p] = rec.t[p] = rec.occ[p];
+    cudaError_t e = cudaMemcpyAsync(tmp + L.off_orbits, orb.data(), sizeof(int4) * orb.size(), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(tmp + L.off_recs, &rec, sizeof(rec), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(tmp + L.total, 0, b_zero, s);
+    tc_wbuild_args a;
+    memset(&a, 0, sizeof(a));
+    a.o = o;
+    a.v = v;
+    const double* zeros = (const double*)(tmp + L.total);
+    a.eps_occ = zeros;  // the epilogue result is discarded; only W is wanted
+    a.eps_vir = zeros;
+    a.t1 = zeros;
+    a.ovov = blocks->ovov;
+    a.recs = (const tc_trip_rec*)(tmp + L.off_recs);
+    a.n_trip = 1;
+    a.partial = (double*)(tmp + L.off_partial);
+    a.n_orbits = L.n_orbits;
+    a.W_debug = W_dev;
+    a.t2_row_stride = O * V * V;
+    if (pad) {
+        double* p_t2 = (double*)(tmp + L.off_t2);
+        double* p_ovoo = (double*)(tmp + L.off_ovoo);
+        double* p_vvvo = (double*)(tmp + L.off_vvvo);
+        for (int x = 0; x < o && e == cudaSuccess; x++) {
+            e = tc_launch_pad_rows(p_t2 + (size_t)x * L.t2row_stride, ldv, t2 + (size_t)x * O * V * V, V, O * V, v, s);
+            if (e == cudaSuccess && (x == i || x == j || x == k))
+                e = tc_launch_pad_rows(p_vvvo + (size_t)x * L.slice_stride, ldv, blocks->vvvo + (size_t)x * V * V * V, V, V * V, v, s);
+        }
+        if (e == cudaSuccess) e = tc_launch_pad_rows(p_ovoo, ldv, blocks->ovoo, V, O * O * O, v, s);
+        a.t2 = p_t2;
+        a.ovoo = p_ovoo;
+        a.slices = p_vvvo;
+        a.slice_stride = L.slice_stride;
+        a.ldv = ldv;
+        a.t2_row_stride = L.t2row_stride;
+    } else {
         a.t2 = t2;
-        a.slice_ptr = (const double* const*)(tmp + b_orb);
-        a.slices_aligned16 = ((uintptr_t)blocks->vvvo % 16 == 0) && (((size_t)v * v * v * sizeof(double)) % 16 == 0);
         a.ovoo = blocks->ovoo;
-        a.ovov = blocks->ovov;
-        a.triplets = (const int4*)(tmp + b_orb + b_sp);
-        a.n_trip = 1;
-        a.partial = (double*)(tmp + b_orb + b_sp + 256);
-        a.n_orbits = (int)orb.size();
-        a.slice_slot = (const int*)(tmp + b_orb + sizeof(double*) * o);
-        a.W_debug = W_dev;
+        a.slices = blocks->vvvo;
+        a.slice_stride = V * V * V;
+        a.ldv = v;
+    }
+    if (e == cudaSuccess) {
         tc_wbuild_maps maps;
-        e = tc_wbuild_make_maps(a, blocks->vvvo, (size_t)v * v * v, o, &maps);
-        if (getenv("TC_FORCE_CPASYNC")) maps.valid = false;
-        if (e == cudaSuccess) e = tc_launch_wbuild(a, &maps, (const int4*)tmp, s);
+        e = tc_wbuild_make_maps(a, o, o, &maps);
+        if (ctx->force_kernel == TC_KERNEL_CPASYNC) maps.valid = false;
+        int ran = 0;
+        if (e == cudaSuccess) e = tc_launch_wbuild(a, &maps, (const int4*)(tmp + L.off_orbits), s, &ran);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        ctx->stats.kernel = ran;
     }
     cudaFree(tmp);
     if (e != cudaSuccess) TC_FAIL(ctx, TC_ERR_CUDA, "debug W kernel failed: %s", cudaGetErrorString(e));

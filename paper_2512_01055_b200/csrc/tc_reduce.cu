@@ -2,6 +2,8 @@
 //   per-unit partials -> S_ijk -> E = sum w_ijk S_ijk, all in a fixed summation order so that two
 //   runs are bit-identical (the paper keeps a sum_ijk array and applies the Kronecker weights
 //   afterwards; same here).
+#include <algorithm>
+
 #include "tc_common.cuh"
 
 namespace {
@@ -9,7 +11,7 @@ namespace {
 __device__ __forceinline__ long long tet(long long i) { return i * (i + 1) * (i + 2) / 6; }
 __device__ __forceinline__ long long tri(long long j) { return j * (j + 1) / 2; }
 
-__global__ void k_make_triplets(int o, long long first, int n, int4* __restrict__ triplets, double* __restrict__ w) {
+__global__ void k_make_triplets(int o, long long first, int n, tc_trip_rec* __restrict__ recs, double* __restrict__ w) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n) return;
     const long long idx = first + t;
@@ -23,8 +25,23 @@ __global__ void k_make_triplets(int o, long long first, int n, int4* __restrict_
     while (tri(j + 1) <= rest) j++;
     while (j > 0 && tri(j) > rest) j--;
     const long long k = rest - tri(j);
-    triplets[t] = make_int4((int)i, (int)j, (int)k, t);
+    // everything resident: slice slot = amplitude-row slot = the occupied index itself
+    int4* out = reinterpret_cast<int4*>(recs + t);
+    out[0] = make_int4((int)i, (int)j, (int)k, t);
+    out[1] = make_int4((int)i, (int)j, (int)k, 0);
+    out[2] = make_int4((int)i, (int)j, (int)k, 0);
     w[t] = 2.0 - (i == j ? 1.0 : 0.0) - (j == k ? 1.0 : 0.0);  // eq. (1): 2 - d_ij - d_jk
+}
+
+// dst[r][c] = src[r][c] for c < v, 0 for v <= c < ldd (zero-padded copy with a 16-byte row stride for TMA)
+__global__ void __launch_bounds__(256) k_pad_rows(double* __restrict__ dst, size_t ldd, const double* __restrict__ src, size_t lds,
+                                                  size_t nrows, int v) {
+    const size_t total = nrows * ldd;
+    for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < total; n += (size_t)gridDim.x * blockDim.x) {
+        const size_t r = n / ldd;
+        const int c = (int)(n - r * ldd);
+        dst[n] = (c < v) ? src[r * lds + c] : 0.0;
+    }
 }
 
 constexpr int RT = 256;
@@ -65,9 +82,9 @@ __global__ void __launch_bounds__(1024) k_reduce_energy(const double* __restrict
 
 }  // namespace
 
-cudaError_t tc_launch_make_triplets(int o, long long first, int n, int4* triplets, double* w, cudaStream_t stream) {
+cudaError_t tc_launch_make_triplets(int o, long long first, int n, tc_trip_rec* recs, double* w, cudaStream_t stream) {
     if (n <= 0) return cudaSuccess;
-    k_make_triplets<<<(n + 255) / 256, 256, 0, stream>>>(o, first, n, triplets, w);
+    k_make_triplets<<<(n + 255) / 256, 256, 0, stream>>>(o, first, n, recs, w);
     return cudaGetLastError();
 }
 
@@ -79,5 +96,13 @@ cudaError_t tc_launch_reduce_units(const double* partial, int n_trip, int n_unit
 
 cudaError_t tc_launch_reduce_energy(const double* S, const double* w, long long n, double* E, cudaStream_t stream) {
     k_reduce_energy<<<1, 1024, 0, stream>>>(S, w, n, E);
+    return cudaGetLastError();
+}
+
+cudaError_t tc_launch_pad_rows(double* dst, size_t ldd, const double* src, size_t lds, size_t nrows, int v, cudaStream_t stream) {
+    if (nrows == 0) return cudaSuccess;
+    const size_t total = nrows * ldd;
+    const unsigned grid = (unsigned)std::min<size_t>((total + 255) / 256, 148 * 16);
+    k_pad_rows<<<grid, 256, 0, stream>>>(dst, ldd, src, lds, nrows, v);
     return cudaGetLastError();
 }

@@ -38,3 +38,12 @@ extern "C" tc_status tc_triplet_decode(int o, long long idx, int* pi, int* pj, i
     if (weight) *weight = 2.0 - (i == j ? 1.0 : 0.0) - (j == k ? 1.0 : 0.0);
     return TC_OK;
 }
+
+// Multi-GPU sharding: contiguous ranges of the linear triplet index, sizes differing by at most one.
+extern "C" tc_status tc_triplet_partition(int o, int world, int rank, long long* first, long long* count) {
+    if (o < 1 || world < 1 || rank < 0 || rank >= world || !first || !count) return TC_ERR_INVALID_ARG;
+    const long long n = tet(o), base = n / world, rem = n % world;
+    *first = rank * base + (rank < rem ? rank : rem);
+    *count = base + (rank < rem ? 1 : 0);
+    return TC_OK;
+}

@@ -107,17 +107,16 @@ k_df_gemm(const double* __restrict__ A, size_t lda, const double* __restrict__ B
 
 }  // namespace
 
+// per device: called by tc_create with the device current
+cudaError_t tc_stager_configure() {
+    cudaError_t e = cudaFuncSetAttribute(k_df_gemm<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_df_gemm<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+}
+
 cudaError_t tc_launch_df_gemm(const double* A, size_t lda, const double* B, size_t ldb, int M, int N, int K,
                               int R2, long long sr1, long long sr2, int C2, long long sc1, long long sc2,
                               double* C, cudaStream_t stream) {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_df_gemm<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_df_gemm<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
     if (M <= 0 || N <= 0 || K <= 0) return cudaSuccess;
     dim3 grid((N + BN - 1) / BN, (M + BM - 1) / BM);
     if (grid.y > 65535) return cudaErrorInvalidConfiguration;

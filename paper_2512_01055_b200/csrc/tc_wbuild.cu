@@ -1,6 +1,8 @@
 // tc_wbuild.cu -- steps a3-a6 of the hot path: the fused W-builder + epilogue, cp.async variant.
-// This is the FALLBACK kernel for problems the TMA path cannot address (odd v: row strides that are
-// not multiples of 16 bytes).  The main path is tc_wbuild_tma.cu; both share tc_wbuild_shared.cuh.
+// This is the FALLBACK kernel for operands the TMA path cannot address: caller arrays whose base pointers are not
+// 16-byte aligned (odd v no longer comes here: the energy calls pad the row length to v + 1 and use TMA).  It is also
+// what tc_debug_force_kernel(TC_KERNEL_CPASYNC) selects, so the tests can compare the two kernels on any input.
+// The main path is tc_wbuild_tma.cu; both share tc_wbuild_shared.cuh.
 //
 // One CTA = one work unit = (occupied triplet i>=j>=k) x (S3-orbit of a virtual tile
 // triple {A,B,C}, A>=B>=C, tile edge T=16).  The CTA forms the up-to-six permuted
@@ -37,10 +39,11 @@ constexpr int B_STAGE = KC * SB;  // doubles
 constexpr int MAX_STEPS = 18;
 
 struct StepDesc {
-    const double* Bp;     // particle B: vvvo[z] + U0*v + V0           (element + k*v*v + n1*v + n2)
-    const double* Bh[2];  // hole B of half h: t2[y or x] + U0*v + V0  (element + l*v*v + n1*v + n2)
-    const double* Ap[2];  // particle A of half h: t2[x][y] (or [y][x]) + W0*v   (element + m*v + d)
-    const double* Ah[2];  // hole A of half h: ovoo[z][x] (or [z][y]) + W0       (element + l*v + m)
+    // ld = row length of the operands (v, or v + 1 for the padded copies)
+    const double* Bp;     // particle B: slice z + U0*ld + V0             (element + k*v*ld + n1*ld + n2)
+    const double* Bh[2];  // hole B of half h: t2 row y or x + U0*ld + V0 (element + l*v*ld + n1*ld + n2)
+    const double* Ap[2];  // particle A of half h: t2[x][y] (or [y][x]) + W0*ld   (element + m*ld + d)
+    const double* Ah[2];  // hole A of half h: ovoo[z][x] (or [z][y]) + W0        (element + l*ld + m)
     int wW, wU, wV;       // valid extents of the m, n1, n2 tiles
     int slot[2];          // shared-memory W tile receiving half h
     int sm[2], sn1[2], sn2[2];  // address strides of m, n1, n2 in that tile (0 for the swizzled last coordinate)
@@ -58,9 +61,9 @@ struct Smem {
 
 // ---- loader: one K chunk of one slab step into a pipeline stage ------------------------------
 template <int VEC>  // VEC = 2: 16-byte cp.async (v even), VEC = 1: 8-byte cp.async (any v)
-__device__ __forceinline__ void issue_chunk(Smem& s, int stage, const StepDesc& d, int phase, int k0, int o, int v) {
+__device__ __forceinline__ void issue_chunk(Smem& s, int stage, const StepDesc& d, int phase, int k0, int o, int v, int ld) {
     const int tid = threadIdx.x;
-    const size_t vv = (size_t)v * v;
+    const size_t vv = (size_t)v * ld;
     const int klim = (phase == 2) ? v : o;
     const double* Bsrc = (phase == 2) ? d.Bp : d.Bh[phase];
     double* Bs = s.B[stage];
@@ -75,7 +78,7 @@ __device__ __forceinline__ void issue_chunk(Smem& s, int stage, const StepDesc& 
         const bool row_ok = (k0 + kk < klim) && (n1 < d.wU);
         int nvalid = d.wV - n2;
         nvalid = row_ok ? (nvalid < 0 ? 0 : (nvalid > VEC ? VEC : nvalid)) : 0;
-        const double* src = nvalid ? Bsrc + (size_t)(k0 + kk) * vv + (size_t)n1 * v + n2 : Bsrc;
+        const double* src = nvalid ? Bsrc + (size_t)(k0 + kk) * vv + (size_t)n1 * ld + n2 : Bsrc;
         const uint32_t dst = smem_u32(Bs + kk * SB + n1 * T + n2);
         if (VEC == 2) cp_async16(dst, src, nvalid * 8);
         else cp_async8(dst, src, nvalid * 8);
@@ -89,7 +92,7 @@ __device__ __forceinline__ void issue_chunk(Smem& s, int stage, const StepDesc& 
             const int h = row >> 4, m = row & 15;
             int nvalid = v - (k0 + kk);
             nvalid = (m < d.wW) ? (nvalid < 0 ? 0 : (nvalid > VEC ? VEC : nvalid)) : 0;
-            const double* src = nvalid ? d.Ap[h] + (size_t)m * v + k0 + kk : d.Ap[h];
+            const double* src = nvalid ? d.Ap[h] + (size_t)m * ld + k0 + kk : d.Ap[h];
             const uint32_t dst = smem_u32(As + row * KC + kk);
             if (VEC == 2) cp_async16(dst, src, nvalid * 8);
             else cp_async8(dst, src, nvalid * 8);
@@ -98,7 +101,7 @@ __device__ __forceinline__ void issue_chunk(Smem& s, int stage, const StepDesc& 
         if (tid < 16 * KC) {
             const int m = tid & 15, kk = tid >> 4;
             const bool ok = (k0 + kk < o) && (m < d.wW);
-            const double* src = ok ? d.Ah[phase] + (size_t)(k0 + kk) * v + m : d.Ah[phase];
+            const double* src = ok ? d.Ah[phase] + (size_t)(k0 + kk) * ld + m : d.Ah[phase];
             cp_async8(smem_u32(As + (phase * 16 + m) * KC + kk), src, ok ? 8 : 0);
         }
     }
@@ -110,17 +113,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_wbuild(const tc_wbuild_args a, 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Smem& s = *reinterpret_cast<Smem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int o = a.o, v = a.v;
+    const int o = a.o, v = a.v, ld = a.ldv;
 
     const int trip = blockIdx.x / a.n_orbits;
     const int orbit = blockIdx.x - trip * a.n_orbits;
-    const int4 tr = a.triplets[trip];
-    const int occ[3] = {tr.x, tr.y, tr.z};
+    const tc_trip_rec rec = a.recs[trip];
+    const int occ[3] = {rec.occ[0], rec.occ[1], rec.occ[2]};
     const int4 ob = orbits[orbit];
     const int bv[3] = {ob.x, ob.y, ob.z};  // tile indices A >= B >= C
     if (occ[0] == occ[1] && occ[1] == occ[2] && !a.W_debug) {
         // weight 2 - d_ij - d_jk = 0 (and S_iii = 0 anyway: R vanishes by symmetry)
-        if (tid == 0) a.partial[(size_t)tr.w * a.n_orbits + orbit] = 0.0;
+        if (tid == 0) a.partial[(size_t)rec.row * a.n_orbits + orbit] = 0.0;
         return;
     }
 
@@ -140,7 +143,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_wbuild(const tc_wbuild_args a, 
             s.slot_of_perm[q] = sop[q];
         }
         int ns = 0;
-        const size_t vv = (size_t)v * v;
+        const size_t vv = (size_t)v * ld;
         for (int q = 0; q < 6; q++) {
             if (sop[q] != q) continue;  // arrangement already covered
             const int pw = c_perm[q][0], pu = c_perm[q][1], pvv = c_perm[q][2];  // which of (A,B,C) is the m / n1 / n2 tile
@@ -150,13 +153,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_wbuild(const tc_wbuild_args a, 
                 const int yp = (zp == 2) ? 1 : 2;
                 const int ox = occ[xp], oy = occ[yp], oz = occ[zp];
                 StepDesc& d = s.steps[ns++];
-                d.Bp = a.slice_ptr[oz] + (size_t)U0 * v + V0;
-                d.Bh[0] = a.t2 + (size_t)oy * o * vv + (size_t)U0 * v + V0;
-                d.Bh[1] = a.t2 + (size_t)ox * o * vv + (size_t)U0 * v + V0;
-                d.Ap[0] = a.t2 + ((size_t)ox * o + oy) * vv + (size_t)W0 * v;
-                d.Ap[1] = a.t2 + ((size_t)oy * o + ox) * vv + (size_t)W0 * v;
-                d.Ah[0] = a.ovoo + ((size_t)oz * o + ox) * o * v + W0;
-                d.Ah[1] = a.ovoo + ((size_t)oz * o + oy) * o * v + W0;
+                const double* t2x = a.t2 + (size_t)rec.t[xp] * a.t2_row_stride;   // amplitude rows by slot
+                const double* t2y = a.t2 + (size_t)rec.t[yp] * a.t2_row_stride;
+                d.Bp = a.slices + (size_t)rec.s[zp] * a.slice_stride + (size_t)U0 * ld + V0;
+                d.Bh[0] = t2y + (size_t)U0 * ld + V0;
+                d.Bh[1] = t2x + (size_t)U0 * ld + V0;
+                d.Ap[0] = t2x + (size_t)oy * vv + (size_t)W0 * ld;
+                d.Ap[1] = t2y + (size_t)ox * vv + (size_t)W0 * ld;
+                d.Ah[0] = a.ovoo + ((size_t)oz * o + ox) * o * ld + W0;
+                d.Ah[1] = a.ovoo + ((size_t)oz * o + oy) * o * ld + W0;
                 d.wW = min(T, v - W0);
                 d.wU = min(T, v - U0);
                 d.wV = min(T, v - V0);
@@ -204,7 +209,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_wbuild(const tc_wbuild_args a, 
         if (ld_c < total) {
             const int phase = (ld_r < nhc) ? 0 : (ld_r < 2 * nhc ? 1 : 2);
             const int k0 = (ld_r - (phase == 0 ? 0 : phase == 1 ? nhc : 2 * nhc)) * KC;
-            issue_chunk<VEC>(s, ld_c % STAGES, s.steps[ld_step], phase, k0, o, v);
+            issue_chunk<VEC>(s, ld_c % STAGES, s.steps[ld_step], phase, k0, o, v, ld);
             ld_c++;
             if (++ld_r == cps) {
                 ld_r = 0;
@@ -301,26 +306,25 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_wbuild(const tc_wbuild_args a, 
     if (tid == 0) {
         double tot = 0.0;
         for (int w = 0; w < NWARPS; w++) tot += s.red[w];
-        a.partial[(size_t)tr.w * a.n_orbits + orbit] = tot;
+        a.partial[(size_t)rec.row * a.n_orbits + orbit] = tot;
     }
 }
 
 }  // namespace
 
+cudaError_t tc_wbuild_cpasync_configure() {
+    cudaError_t e = cudaFuncSetAttribute(k_wbuild<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_wbuild<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+}
+
 cudaError_t tc_launch_wbuild_cpasync(const tc_wbuild_args& a, const int4* orbits, cudaStream_t stream) {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_wbuild<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_wbuild<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
     const long long nblocks = (long long)a.n_trip * a.n_orbits;
     if (nblocks <= 0) return cudaSuccess;
     if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    // 16-byte cp.async needs 16-byte aligned rows: v even and 16-byte aligned base pointers
-    const bool vec2 = (a.v % 2 == 0) && (((uintptr_t)a.t2 | (uintptr_t)a.ovoo) % 16 == 0) && a.slices_aligned16;
+    // 16-byte cp.async needs 16-byte aligned rows: even row length and strides, 16-byte aligned base pointers
+    const bool vec2 = (a.ldv % 2 == 0) && (a.slice_stride % 2 == 0) && (a.t2_row_stride % 2 == 0) &&
+                      (((uintptr_t)a.t2 | (uintptr_t)a.ovoo | (uintptr_t)a.slices) % 16 == 0);
     if (vec2) k_wbuild<2><<<(unsigned)nblocks, NTHREADS, sizeof(Smem), stream>>>(a, orbits);
     else k_wbuild<1><<<(unsigned)nblocks, NTHREADS, sizeof(Smem), stream>>>(a, orbits);
     return cudaGetLastError();

@@ -26,6 +26,7 @@
 // CTA order: tile orbit slow, triplet fast (L2 reuse of the I_i and I_j slabs between concurrent CTAs).
 #include <type_traits>
 
+#include "tc_tma.cuh"
 #include "tc_wbuild_shared.cuh"
 
 namespace {
@@ -50,6 +51,7 @@ struct Step {
     int U0, V0, W0;  // first virtual index of the n1, n2 and m tiles
     int ox, oy, oz;  // occupied indices in the roles x, y, z
     int zslot;       // slot of slice oz in the slice array
+    int tsx, tsy;    // slots of the amplitude rows t2[ox], t2[oy]
     int nxb, ny, nz; // 8-blocks with at least one index below v: rows, n1, n2 (1 or 2)
     int slot[2];     // shared-memory W tile receiving half h
     int sm[2], sn1[2], sn2[2];  // address strides of m, n1, n2 in that tile (0 for the rotated last coordinate)
@@ -67,76 +69,16 @@ struct __align__(128) Smem {
     int nsteps;
 };
 
-// ---- mbarrier / TMA primitives -----------------------------------------------------------
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t done;
-    do {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n"
-            : "=r"(done)
-            : "r"(bar), "r"(parity)
-            : "memory");
-    } while (!done);
-}
-// keeps a loop-invariant address in a register (the compiler otherwise rematerialises the
-// shared-window base from special registers at every use)
-__device__ __forceinline__ uint32_t opaque(uint32_t x) {
-    asm volatile("mov.u32 %0, %0;" : "+r"(x));
-    return x;
-}
-__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(dst),
-        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
-        : "memory");
-}
-__device__ __forceinline__ bool elect_one() {
-    uint32_t pred;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "elect.sync _|p, 0xffffffff;\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(pred));
-    return pred != 0;
-}
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory"); }
 
-#ifdef TCW_TRACE
-// Timeline instrumentation of one CTA (development builds only).
-constexpr int TRACE_N = 2048;
-__device__ long long g_trace[8][TRACE_N];
-#ifndef TCW_TRACE_CTA
-#define TCW_TRACE_CTA 3000
-#endif
-#define TRACE(row, idx, cond) do { if (blockIdx.x == TCW_TRACE_CTA && (cond) && (idx) < TRACE_N) g_trace[row][idx] = clock64(); } while (0)
-#else
-#define TRACE(row, idx, cond) do { } while (0)
-#endif
 
 struct ConsumerState {
-    int tcount;       // chunks consumed so far (timeline instrumentation)
     int stage;        // ring position of the next chunk to consume
     uint32_t parity;  // its full-barrier parity
     int lane;
     int nhc, npc;     // chunks per hole phase / of the particle phase
     uint32_t full0, empty0;  // shared addresses of full[0] / empty[0]
     uint32_t bB, bAp, bAh;   // this thread's fragment addresses in stage 0 (B, particle A, hole A)
-    bool warp0, warp5;       // timeline instrumentation: is this consumer warp 0 / 5
     bool skew;               // second warp of its scheduler (warps w and w+4 share one)
     // deferred flush of the previous step's half 1 (rows 16-31): folded into the W tile under the hole phase of
     // half 0, whose chunks carry only half the DMMAs and leave the warp idle most of the time
@@ -150,14 +92,6 @@ struct ConsumerState {
     int fr, fk, warp;        // place of this thread in the DMMA C fragment / of its warp in the column tile
 };
 
-__device__ __forceinline__ double lds64(uint32_t addr) {
-    double x;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(x) : "r"(addr));
-    return x;
-}
-__device__ __forceinline__ void sts64(uint32_t addr, double x) {
-    asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(x) : "memory");
-}
 __device__ __forceinline__ void cons_advance(ConsumerState& cs) {
     if (++cs.stage == STAGES) {
         cs.stage = 0;
@@ -239,9 +173,7 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], double (&hol
             cs.pend_on = false;
         }
         for (int r = 0; r < cs.nhc; r++) {
-            TRACE(4, cs.tcount, cs.lane == 0 && cs.warp0);
             mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
-            TRACE(5, cs.tcount, cs.lane == 0 && cs.warp0);
             const uint32_t pa = cs.bAh + cs.stage * AST + (2 * h) * 256;
             const uint32_t pb = cs.bB + cs.stage * BST;
             double fa[NXB], fb[NY][NZ];
@@ -260,9 +192,6 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], double (&hol
             cons_release(cs, cs.stage);
             if (h == 0 && cs.pend_on && r < 4) flush_slice_n(r);
             if (h == 1 && cs.pend0_on && r < 4) flush_hold_n(r);
-            TRACE(6, cs.tcount, cs.lane == 0 && cs.warp0);
-            TRACE(7, cs.tcount, cs.lane == 0 && cs.warp5);
-            cs.tcount++;
             cons_advance(cs);
         }
     }
@@ -292,9 +221,7 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], double (&hol
         while (clock64() - t0 < 150) {}
     }
     for (int r = 0; r < cs.npc; r++) {
-        TRACE(4, cs.tcount, cs.lane == 0 && cs.warp0);
         mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
-        TRACE(5, cs.tcount, cs.lane == 0 && cs.warp0);
         const uint32_t pa = cs.bAp + cs.stage * AST;
         const uint32_t pb = cs.bB + cs.stage * BST;
         double fa[2][NXB], fb[NY][NZ];
@@ -316,9 +243,6 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], double (&hol
                     for (int z = 0; z < NZ; z++) dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[h][xb], fb[y][z]);
         // every DMMA that reads this chunk's fragments has been issued (operands are read at issue)
         cons_release(cs, cs.stage);
-        TRACE(6, cs.tcount, cs.lane == 0 && cs.warp0);
-        TRACE(7, cs.tcount, cs.lane == 0 && cs.warp5);
-        cs.tcount++;
         cons_advance(cs);
     }
 }
@@ -332,26 +256,20 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     Smem& s = *reinterpret_cast<Smem*>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int o = a.o, v = a.v;
-    TRACE(0, TRACE_N - 1, tid == 0);   // kernel entry
 
     // CTA order: tile orbit slow, triplet fast.  CTAs that run together then work on the same orbit for
     // consecutive triplets (i, j, k), (i, j, k+1), ...: they walk the same step sequence and share the slabs of
     // the slices I_i and I_j (12 of a unit's 18 slabs) in L2; with the triplet slow and the orbit fast,
     // neighbours share two tiles and hence only 6 of 18.
-#ifdef TCW_ORBIT_FAST
-    const int trip = blockIdx.x / a.n_orbits;
-    const int orbit = blockIdx.x - trip * a.n_orbits;
-#else
     const int orbit = blockIdx.x / a.n_trip;
     const int trip = blockIdx.x - orbit * a.n_trip;
-#endif
-    const int4 tr = a.triplets[trip];
-    const int occ[3] = {tr.x, tr.y, tr.z};
+    const tc_trip_rec rec = a.recs[trip];
+    const int occ[3] = {rec.occ[0], rec.occ[1], rec.occ[2]};
     const int4 ob = orbits[orbit];
     const int bv[3] = {ob.x, ob.y, ob.z};  // tile indices A >= B >= C
     if (occ[0] == occ[1] && occ[1] == occ[2] && !a.W_debug) {
         // weight 2 - d_ij - d_jk = 0 (and S_iii = 0 anyway: R vanishes by symmetry)
-        if (tid == 0) a.partial[(size_t)tr.w * a.n_orbits + orbit] = 0.0;
+        if (tid == 0) a.partial[(size_t)rec.row * a.n_orbits + orbit] = 0.0;
         return;
     }
 
@@ -384,7 +302,9 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             d.ox = occ[xp];
             d.oy = occ[yp];
             d.oz = occ[zp];
-            d.zslot = a.slice_slot[occ[zp]];
+            d.zslot = rec.s[zp];
+            d.tsx = rec.t[xp];
+            d.tsy = rec.t[yp];
             d.nxb = (v - d.W0 > 8) ? 2 : 1;
             d.ny = (v - d.U0 > 8) ? 2 : 1;
             d.nz = (v - d.V0 > 8) ? 2 : 1;
@@ -448,7 +368,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             const int st = seg_i / 3, ph = seg_i - 3 * st;
             const Step& d = s.steps[st];
             if (ph < 2) {  // hole phase of half ph: B = t2[y or x][l][n1][n2], A = ovoo[z][x or y][l][m]
-                const int yy = ph ? d.ox : d.oy, xx = ph ? d.oy : d.ox;
+                const int yy = ph ? d.tsx : d.tsy, xx = ph ? d.oy : d.ox;   // B: amplitude row of y (by slot), A: (ov|oo) of x
                 g.n = nhc;
                 g.kdim = 1;
                 g.tx = d.nz * B_BOX_BYTES + d.nxb * AH_BOX_BYTES;
@@ -475,7 +395,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 } else {
                     g.map = &mapT2p;
                     g.kdim = 0;
-                    g.c0 = 0; g.c1 = d.W0; g.c2 = (pw == 2) ? d.oy : d.ox; g.c3 = (pw == 2) ? d.ox : d.oy;
+                    g.c0 = 0; g.c1 = d.W0; g.c2 = (pw == 2) ? d.oy : d.ox; g.c3 = (pw == 2) ? d.tsx : d.tsy;
                     g.dst0 = A0 + (pw - 2) * AP_BOX_BYTES; g.dst_stride = A_STAGE * 8;
                     g.active = true;
                 }
@@ -483,7 +403,6 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         };
         const int nseg = 3 * nsteps;
         int stage = 0;
-        int tchunk = 0;     // chunks issued so far (timeline instrumentation)
         uint32_t wrap = 0;  // how many times the ring has wrapped
         for (int seg_i = 0; seg_i < nseg; seg_i++) {
             Seg g;
@@ -492,16 +411,11 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 // every stream waits, active or not: a stream that ran ahead by two ring turns would
                 // alias the barrier's phase parity
                 if (wrap > 0) mbar_wait(empty0 + stage * 8, (wrap - 1) & 1);
-                TRACE(0, tchunk, leader && pw == 0);
-                TRACE(2, tchunk, leader && pw == 1);
-                TRACE(3, tchunk, leader && pw == 2);
                 if (leader) {
                     const uint32_t full = full0 + stage * 8;
                     if (pw == 0) mbar_expect_tx(full, g.tx);
                     if (g.active) tma_load_4d(g.dst0 + stage * g.dst_stride, g.map, g.kdim == 0 ? r * KC : g.c0, g.kdim == 1 ? r * KC : g.c1, g.c2, g.c3, full);
                 }
-                TRACE(1, tchunk, leader && pw == 0);
-                tchunk++;
                 if (++stage == STAGES) {
                     stage = 0;
                     wrap++;
@@ -520,9 +434,6 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     cs.stage = 0;
     cs.parity = 0;
     cs.lane = lane;
-    cs.tcount = 0;
-    cs.warp0 = (warp == 0);
-    cs.warp5 = (warp == 5);
     cs.skew = (warp & 4) != 0;
     cs.pend_on = false;
     cs.pend0_on = false;
@@ -572,6 +483,10 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         // Half 1 can wait: the next step's first phase (hole, half 0) touches rows 0-15 only, so rows 16-31 are
         // folded into their tile under it, four accumulators per hole chunk (see run_step).  Not when the two halves
         // share a tile (they need the barrier between them) and not for very short steps (ring-ordering argument).
+        // The ring-ordering argument needs cps >= nhc + 2*4 (the pending halves are folded in under the first four
+        // chunks of each hole phase and must be done before a warp can be STAGES chunks ahead): cps = 2 nhc + npc >= 16
+        // gives it for every o (npc >= 16 - 2 nhc  =>  cps - nhc - 8 = nhc + npc - 8 >= 0 when cps >= 16, nhc >= 1).
+        static_assert(STAGES == 3, "the defer threshold below (cps >= 16) was derived for a 3-stage ring and a 4-chunk flush window");
         const bool defer = (cps >= 16) && (d.slot[0] != d.slot[1]);
         if (defer) {   // park half 0 in spare registers: nothing of the flush is left on the critical path
 #pragma unroll
@@ -670,7 +585,6 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     }
     consumer_bar();
 
-    TRACE(1, TRACE_N - 1, tid == 0);   // main loop done, epilogue starts
     if (a.W_debug) tcw::dump_W(s.tiles, s.slot_of_perm, bv, v, a.W_debug, tid, NCONS);
     double sum = tcw::orbit_energy(s.tiles, s.slot_of_perm, bv, occ, a, tid, NCONS);
 #pragma unroll
@@ -680,77 +594,43 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     if (tid == 0) {
         double tot = 0.0;
         for (int w = 0; w < NCONS_WARPS; w++) tot += s.red[w];
-        a.partial[(size_t)tr.w * a.n_orbits + orbit] = tot;
+        a.partial[(size_t)rec.row * a.n_orbits + orbit] = tot;
     }
-    TRACE(2, TRACE_N - 1, tid == 0);   // unit done
-}
-
-// ---- host: tensor maps -----------------------------------------------------------------------
-typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                              const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-encode_fn get_encode() {
-    static encode_fn fn = nullptr;
-    if (!fn) {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (encode_fn)p;
-    }
-    return fn;
-}
-
-// rank-4 FP64 map; dims/strides innermost first (stride of dim 0 is implicit), strides in doubles
-bool encode4(CUtensorMap* m, const double* base, const cuuint64_t dim[4], const cuuint64_t stride_dbl[3], const cuuint32_t box[4]) {
-    encode_fn fn = get_encode();
-    if (!fn) return false;
-    cuuint64_t strides[3] = {stride_dbl[0] * 8, stride_dbl[1] * 8, stride_dbl[2] * 8};
-    cuuint32_t estr[4] = {1, 1, 1, 1};
-    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)base, dim, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 }  // namespace
 
-#ifdef TCW_TRACE
-extern "C" int tc_debug_read_trace(long long* out) {
-    return (int)cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * 8 * TRACE_N);
-}
-#endif
-
-cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, const double* slice_base, size_t slice_stride, int nslots,
-                                tc_wbuild_maps* out) {
+cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, int nslots, int n_tslots, tc_wbuild_maps* out) {
     out->valid = false;
-    const cuuint64_t o = a.o, v = a.v;
-    // TMA needs 16-byte aligned bases and strides: v even, aligned pointers
-    if (v % 2 != 0 || slice_stride % 2 != 0 || nslots < 1) return cudaSuccess;
-    if ((((uintptr_t)a.t2) | ((uintptr_t)a.ovoo) | ((uintptr_t)slice_base)) % 16 != 0) return cudaSuccess;
+    const cuuint64_t o = a.o, v = a.v, ld = a.ldv;
+    // TMA needs 16-byte aligned bases and strides.  Odd v never gets here unpadded: the energy calls pass zero-padded
+    // copies with ldv = v + 1, so only caller pointers that are not 16-byte aligned take the cp.async kernel.
+    if (ld % 2 != 0 || a.slice_stride % 2 != 0 || a.t2_row_stride % 2 != 0 || nslots < 1 || n_tslots < 1) return cudaSuccess;
+    if ((((uintptr_t)a.t2) | ((uintptr_t)a.ovoo) | ((uintptr_t)a.slices)) % 16 != 0) return cudaSuccess;
     bool ok = true;
     {   // slices [slot][d][b][c] viewed as dims (c, d, b, slot)
         const cuuint64_t dim[4] = {v, v, v, (cuuint64_t)nslots};
-        const cuuint64_t str[3] = {v * v, v, (cuuint64_t)slice_stride};
+        const cuuint64_t str[3] = {v * ld, ld, (cuuint64_t)a.slice_stride};
         const cuuint32_t box[4] = {8, KC, 16, 1};
-        ok = ok && encode4(&out->I, slice_base, dim, str, box);
+        ok = ok && tctma::encode4(&out->I, a.slices, dim, str, box);
     }
-    {   // t2[y][l][n1][n2] viewed as dims (n2, l, n1, y)
-        const cuuint64_t dim[4] = {v, o, v, o};
-        const cuuint64_t str[3] = {v * v, v, o * v * v};
+    {   // t2[tslot][l][n1][n2] viewed as dims (n2, l, n1, tslot)
+        const cuuint64_t dim[4] = {v, o, v, (cuuint64_t)n_tslots};
+        const cuuint64_t str[3] = {v * ld, ld, (cuuint64_t)a.t2_row_stride};
         const cuuint32_t box[4] = {8, KC, 16, 1};
-        ok = ok && encode4(&out->T2h, a.t2, dim, str, box);
+        ok = ok && tctma::encode4(&out->T2h, a.t2, dim, str, box);
     }
-    {   // t2[x][y][m][d] as dims (d, m, y, x)
-        const cuuint64_t dim[4] = {v, v, o, o};
-        const cuuint64_t str[3] = {v, v * v, o * v * v};
+    {   // t2[tslot][y][m][d] as dims (d, m, y, tslot)
+        const cuuint64_t dim[4] = {v, v, o, (cuuint64_t)n_tslots};
+        const cuuint64_t str[3] = {ld, v * ld, (cuuint64_t)a.t2_row_stride};
         const cuuint32_t box[4] = {KC, 16, 1, 1};
-        ok = ok && encode4(&out->T2p, a.t2, dim, str, box);
+        ok = ok && tctma::encode4(&out->T2p, a.t2, dim, str, box);
     }
     {   // ovoo[z][x][l][m] as dims (m, l, x, z)
         const cuuint64_t dim[4] = {v, o, o, o};
-        const cuuint64_t str[3] = {v, o * v, o * o * v};
+        const cuuint64_t str[3] = {ld, o * ld, o * o * ld};
         const cuuint32_t box[4] = {8, KC, 1, 1};
-        ok = ok && encode4(&out->Ovoo, a.ovoo, dim, str, box);
+        ok = ok && tctma::encode4(&out->Ovoo, a.ovoo, dim, str, box);
     }
     out->valid = ok;
     return cudaSuccess;
@@ -762,18 +642,23 @@ int tc_wbuild_num_orbits(int v) {
     return (int)(nb * (nb + 1) * (nb + 2) / 6);
 }
 
-cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const tc_wbuild_maps* maps, const int4* orbits, cudaStream_t stream) {
-    if (!maps || !maps->valid) return tc_launch_wbuild_cpasync(a, orbits, stream);
-    static bool configured = false;
-    constexpr int kSmem = (int)sizeof(Smem) + 128;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_wbuild_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
-        if (e != cudaSuccess) return e;
-        configured = true;
+constexpr int kSmemTma = (int)sizeof(Smem) + 128;
+
+// per device: called by tc_create with the device current (the attribute is per device, not per process)
+cudaError_t tc_wbuild_configure() {
+    return cudaFuncSetAttribute(k_wbuild_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemTma);
+}
+
+cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const tc_wbuild_maps* maps, const int4* orbits, cudaStream_t stream,
+                             int* kernel_out) {
+    if (!maps || !maps->valid) {
+        if (kernel_out) *kernel_out = TC_KERNEL_CPASYNC;
+        return tc_launch_wbuild_cpasync(a, orbits, stream);
     }
+    if (kernel_out) *kernel_out = TC_KERNEL_TMA;
     const long long nblocks = (long long)a.n_trip * a.n_orbits;
     if (nblocks <= 0) return cudaSuccess;
     if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    k_wbuild_tma<<<(unsigned)nblocks, NTHREADS, kSmem, stream>>>(a, orbits, maps->I, maps->T2h, maps->T2p, maps->Ovoo);
+    k_wbuild_tma<<<(unsigned)nblocks, NTHREADS, kSmemTma, stream>>>(a, orbits, maps->I, maps->T2h, maps->T2p, maps->Ovoo);
     return cudaGetLastError();
 }

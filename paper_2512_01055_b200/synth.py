@@ -2,9 +2,10 @@
 
 This module is shared by the oracle's tests and by the CUDA path's tests and
 bench.  It holds NO arithmetic of the (T) method itself: it only draws the
-problem inputs (DF factors, orbital energies, amplitudes) and derives the
-integral blocks the boundary accepts.  It imports neither ``oracle`` nor the
-CUDA binding.
+problem inputs (DF factors, orbital energies, MP2 amplitudes).  The integral
+blocks of eq. (6) -- step a2 of the method -- are NOT derived here: the oracle
+side builds them in ``oracle/blocks.py``, the CUDA side in ``csrc/tc_stager.cu``.
+It imports neither ``oracle`` nor the CUDA binding.
 
 Recipe (BASELINE.json ``configs``):
 
@@ -47,6 +48,9 @@ CONFIGS = {
     "cfg2": (40, 400, 1200, 2),
     "cfg3": (60, 500, 1500, 3),
     "cfg4": (100, 800, 2400, 4),
+    # the paper's own shape, v/o ~ 4 -- sized like (H2O)14 / cc-pVDZ (336 AOs, PAPER.md:77-83,
+    # Table 1; o and v are inferred, the paper does not print them); v = 266 = 16*16 + 10 is ragged
+    "h2o14": (70, 266, 800, 5),
 }
 
 
@@ -93,7 +97,8 @@ class Problem:
       Boo[Q][i][j], Bov[Q][i][a], Bvv[Q][a][b];
       t1[i][a]; t2[i][j][a][b] = t_ij^ab;
       vvvo[x][d][b][c] = (bd|cx); ovoo[j][k][l][c] = (lj|kc); ovov[j][k][b][c] = (jb|kc).
-    The integral blocks are optional (None until ``materialise_blocks``).
+    The integral blocks are optional: None here; the tests fill them on the oracle side
+    (``oracle.blocks.materialise_blocks``) or on the device (``tc_build_blocks``).
     """
     o: int
     v: int
@@ -131,7 +136,7 @@ def mp2_amplitudes(Bov: np.ndarray, eps_occ: np.ndarray, eps_vir: np.ndarray) ->
 
 
 def make_problem(o: int, v: int, naux: int, seed: int, sigma_B: float = 0.05,
-                 sigma_t1: float = 0.01, blocks: bool = False, with_t2: bool = True) -> Problem:
+                 sigma_t1: float = 0.01, with_t2: bool = True) -> Problem:
     """Draw one synthetic problem with the BASELINE.json recipe.  with_t2=False leaves ``t2`` None (the
     caller derives the MP2 amplitudes on the device with ``mp2_amplitudes_device``: at cfg4 size ``t2`` is 51 GB)."""
     N = o + v
@@ -148,10 +153,7 @@ def make_problem(o: int, v: int, naux: int, seed: int, sigma_B: float = 0.05,
     t1 = counter_normal(seed, TENSOR_T1, np.arange(o * v), sigma_t1).reshape(o, v)
     Boo, Bov, Bvv = _split_B(B, o)
     t2 = mp2_amplitudes(Bov, eps_occ, eps_vir) if with_t2 else None
-    prob = Problem(o, v, naux, eps_occ, eps_vir, np.ascontiguousarray(t1), t2, Boo, Bov, Bvv)
-    if blocks:
-        materialise_blocks(prob)
-    return prob
+    return Problem(o, v, naux, eps_occ, eps_vir, np.ascontiguousarray(t1), t2, Boo, Bov, Bvv)
 
 
 def mp2_amplitudes_device(Bov, eps_occ, eps_vir):
@@ -178,6 +180,93 @@ def mp2_amplitudes_device(Bov, eps_occ, eps_vir):
     return t2
 
 
+def mp2_amplitude_rows(Bov: np.ndarray, eps_occ: np.ndarray, eps_vir: np.ndarray, rows) -> np.ndarray:
+    """``mp2_amplitudes`` restricted to the first occupied index in ``rows``: returns an (o, o, v, v) array whose rows
+    t2[x] (x in rows) hold t_xl^ab for all l and whose other rows are untouched zeros (the array is calloc-backed, so
+    at cfg4 size -- 51 GB in full -- only the requested rows cost memory)."""
+    naux, o, v = Bov.shape
+    Bflat = Bov.reshape(naux, o * v)
+    t2 = np.zeros((o, o, v, v))
+    ea = eps_vir.reshape(v, 1, 1)
+    eb = eps_vir.reshape(1, 1, v)
+    el = eps_occ.reshape(1, o, 1)
+    for x in rows:
+        Bx = np.ascontiguousarray(Bov[:, x, :])
+        g1 = (Bx.T @ Bflat).reshape(v, o, v)                       # (xa|lb)  [a][l][b]
+        g2 = (Bflat.T @ Bx).reshape(o, v, v).transpose(2, 0, 1)    # (lb|xa)  [a][l][b]
+        d1 = eps_occ[x] - ea + el - eb                             # e_x - e_a + e_l - e_b
+        d2 = el - eb + eps_occ[x] - ea                             # e_l - e_b + e_x - e_a
+        t2[x] = (0.5 * (g1 / d1 + g2 / d2)).transpose(1, 0, 2)     # [l][a][b]
+    return t2
+
+
+def _splitmix64_torch(x):
+    """``_splitmix64`` on int64 tensors (two's-complement wrap-around = uint64 arithmetic; logical shifts by masking)."""
+    import torch
+
+    def lsr(z, n):
+        return (z >> n) & ((1 << (64 - n)) - 1)
+
+    def c(u):   # uint64 constant as the int64 with the same bits
+        return u - (1 << 64) if u >= (1 << 63) else u
+
+    z = x + c(_GOLD)
+    z = (z ^ lsr(z, 30)) * c(_MIX1)
+    z = (z ^ lsr(z, 27)) * c(_MIX2)
+    return z ^ lsr(z, 31)
+
+
+def counter_normal_torch(seed: int, tensor_id: int, idx, sigma: float):
+    """``counter_normal`` with torch tensors (idx: int64 tensor on any device): the same counters and the same
+    Box-Muller formula, so every element agrees with the numpy generator up to the last bits of log/cos."""
+    import torch
+    base = ((seed * _GOLD) & 0xFFFFFFFFFFFFFFFF) ^ ((tensor_id * _MIX1) & 0xFFFFFFFFFFFFFFFF)
+    base = base - (1 << 64) if base >= (1 << 63) else base
+    ctr = 2 * idx + base
+    r1 = _splitmix64_torch(ctr)
+    r2 = _splitmix64_torch(ctr + 1)
+    scale = 1.0 / 9007199254740992.0
+    u1 = (((r1 >> 11) & ((1 << 53) - 1)).double() + 1.0) * scale
+    u2 = ((r2 >> 11) & ((1 << 53) - 1)).double() * scale
+    return sigma * torch.sqrt(-2.0 * torch.log(u1)) * torch.cos(2.0 * np.pi * u2)
+
+
+def make_problem_device(o: int, v: int, naux: int, seed: int, device="cuda", sigma_B: float = 0.05, sigma_t1: float = 0.01):
+    """``make_problem`` with the DF factors drawn on the device (bench.py's throughput legs at sizes where the host draw
+    of B -- 15 GB at cfg4 -- would take minutes): dict of device tensors eps_occ, eps_vir, t1, t2, Boo, Bov, Bvv.
+    Same counter-based recipe; values agree with ``make_problem`` up to the last bits of log/cos."""
+    import torch
+    N = o + v
+    p = torch.arange(N, dtype=torch.int64, device=device)
+    lo = torch.minimum(p[:, None], p[None, :])
+    hi = torch.maximum(p[:, None], p[None, :])
+    pair = lo * N + hi
+    Boo = torch.empty((naux, o, o), dtype=torch.float64, device=device)
+    Bov = torch.empty((naux, o, v), dtype=torch.float64, device=device)
+    Bvv = torch.empty((naux, v, v), dtype=torch.float64, device=device)
+    step = max(1, min(naux, (1 << 25) // (N * N)))
+    for q0 in range(0, naux, step):
+        q1 = min(naux, q0 + step)
+        Q = torch.arange(q0, q1, dtype=torch.int64, device=device)[:, None, None]
+        B = counter_normal_torch(seed, TENSOR_B, Q * (N * N) + pair[None], sigma_B)
+        Boo[q0:q1] = B[:, :o, :o]
+        Bov[q0:q1] = B[:, :o, o:]
+        Bvv[q0:q1] = B[:, o:, o:]
+        del B
+    ho = make_small_host(o, v, seed, sigma_t1)
+    d = {k: torch.from_numpy(x).to(device) for k, x in ho.items()}
+    d.update(Boo=Boo, Bov=Bov, Bvv=Bvv)
+    d["t2"] = mp2_amplitudes_device(Bov, d["eps_occ"], d["eps_vir"])
+    return d
+
+
+def make_small_host(o: int, v: int, seed: int, sigma_t1: float = 0.01):
+    """eps_occ, eps_vir, t1 of the recipe (host numpy)."""
+    return {"eps_occ": counter_uniform(seed, TENSOR_EPS_OCC, np.arange(o), -2.0, -0.3),
+            "eps_vir": counter_uniform(seed, TENSOR_EPS_VIR, np.arange(v), 0.1, 5.0),
+            "t1": np.ascontiguousarray(counter_normal(seed, TENSOR_T1, np.arange(o * v), sigma_t1).reshape(o, v))}
+
+
 def config_sizes(name: str):
     """(o, v, naux, seed) of a named BASELINE.json config, or of an ad-hoc "o,v,naux,seed" string."""
     if name in CONFIGS:
@@ -186,13 +275,12 @@ def config_sizes(name: str):
     return o, v, naux, seed
 
 
-def make_config(name: str, blocks: bool = False, sigma_B: float = 0.05, with_t2: bool = True) -> Problem:
+def make_config(name: str, sigma_B: float = 0.05, with_t2: bool = True) -> Problem:
     o, v, naux, seed = config_sizes(name)
-    return make_problem(o, v, naux, seed, sigma_B=sigma_B, blocks=blocks, with_t2=with_t2)
+    return make_problem(o, v, naux, seed, sigma_B=sigma_B, with_t2=with_t2)
 
 
-def closed_form_problem(o: int, v: int, naux: int, blocks: bool = True,
-                        t1_zero: bool = False) -> Problem:
+def closed_form_problem(o: int, v: int, naux: int, t1_zero: bool = False) -> Problem:
     """Closed-form inputs of the worked examples:
     B^Q_pq = 0.3 cos(0.7(Q+1) + 1.3(p+q) + 0.11 p q) / (1 + 0.1|p-q|),
     eps_occ[i] = -1.5 + 0.35 i, eps_vir[a] = 0.4 + 0.45 a,
@@ -211,30 +299,4 @@ def closed_form_problem(o: int, v: int, naux: int, blocks: bool = True,
         t1 = np.zeros_like(t1)
     Boo, Bov, Bvv = _split_B(B, o)
     t2 = mp2_amplitudes(Bov, eps_occ, eps_vir)
-    prob = Problem(o, v, naux, eps_occ, eps_vir, np.ascontiguousarray(t1), t2, Boo, Bov, Bvv)
-    if blocks:
-        materialise_blocks(prob)
-    return prob
-
-
-def vvvo_slice(prob: Problem, x: int) -> np.ndarray:
-    """I_x[d][b][c] = (bd|cx) for one occupied index x (v^3 doubles)."""
-    naux, v = prob.naux, prob.v
-    A = prob.Bvv.reshape(naux, v * v)                 # [Q][(d,b)] (Bvv is symmetric)
-    return (A.T @ prob.Bov[:, x, :]).reshape(v, v, v)
-
-
-def materialise_blocks(prob: Problem) -> Problem:
-    """Fill vvvo / ovoo / ovov from the DF factors (input preparation only)."""
-    o, v, naux = prob.o, prob.v, prob.naux
-    vvvo = np.empty((o, v, v, v), dtype=np.float64)
-    for x in range(o):
-        vvvo[x] = vvvo_slice(prob, x)
-    # ovoo[j][k][l][c] = (lj|kc) = sum_Q Boo[Q][l][j] Bov[Q][k][c]
-    ovoo = np.einsum("qlj,qkc->jklc", prob.Boo, prob.Bov, optimize=True)
-    # ovov[j][k][b][c] = (jb|kc) = sum_Q Bov[Q][j][b] Bov[Q][k][c]
-    ovov = np.einsum("qjb,qkc->jkbc", prob.Bov, prob.Bov, optimize=True)
-    prob.vvvo = vvvo
-    prob.ovoo = np.ascontiguousarray(ovoo)
-    prob.ovov = np.ascontiguousarray(ovov)
-    return prob
+    return Problem(o, v, naux, eps_occ, eps_vir, np.ascontiguousarray(t1), t2, Boo, Bov, Bvv)

@@ -7,8 +7,12 @@ relative error <= 1e-9; on inputs whose |E| is far above 1 Eh only the relative 
 import numpy as np
 import pytest
 
+import harness
 import oracle
+from paper_2512_01055_b200 import binding as binding_mod
 from paper_2512_01055_b200 import synth
+
+from paper_2512_01055_b200.binding import TC_KERNEL_AUTO, TC_KERNEL_CPASYNC, TC_KERNEL_TMA
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -44,7 +48,7 @@ class DevProblem:
         return (self.p.naux, self.Boo, self.Bov, self.Bvv)
 
 
-def run_slice(ctx, dp, first, count, use_df=False):
+def run_slice(ctx, dp, first, count, use_df=False, expect_kernel=None):
     p = dp.p
     nb = ctx.workspace_bytes(p.o, p.v, p.naux if use_df else 0)
     ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
@@ -52,7 +56,18 @@ def run_slice(ctx, dp, first, count, use_df=False):
     kw = dict(df=dp.df()) if use_df else dict(blocks=dp.blocks())
     E = ctx.triples_energy_slice(p.o, p.v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, workspace=ws, workspace_bytes=nb,
                                  first=first, count=count, S_dev=S, **kw)
+    if expect_kernel is not None and count > 0:
+        assert ctx.get_stats()["kernel"] == expect_kernel, ctx.get_stats()
     return E, S.cpu().numpy()[:count]
+
+
+def hole_chunks(o):
+    return (o + 3) // 4
+
+
+def chunks_per_step(o, v):
+    """cps of csrc/tc_wbuild_tma.cu: the deferred flush is taken when cps >= 16."""
+    return 2 * hole_chunks(o) + (v + 3) // 4
 
 
 def assert_energy(E, E_ref):
@@ -63,9 +78,10 @@ def assert_energy(E, E_ref):
 
 
 # ---- W alone (steps a3 + a4), any order of i, j, k ------------------------------------------
-@pytest.mark.parametrize("o,v,naux,seed", [(3, 4, 5, 11), (4, 19, 7, 12), (5, 37, 9, 13), (3, 48, 6, 14)])
+# (5,64) and (9,50): deferred-flush sizes with 2 and 3 hole chunks, the second with ragged tiles (50 = 3*16 + 2)
+@pytest.mark.parametrize("o,v,naux,seed", [(3, 4, 5, 11), (4, 19, 7, 12), (5, 37, 9, 13), (3, 48, 6, 14), (5, 64, 8, 15), (9, 50, 10, 16)])
 def test_W_matches_oracle(ctx, o, v, naux, seed):
-    p = synth.make_problem(o, v, naux, seed, sigma_B=0.3, blocks=True)
+    p = harness.make_problem(o, v, naux, seed, sigma_B=0.3, blocks=True)
     dp = DevProblem(p)
     rng = np.random.default_rng(seed)
     trips = [(o - 1, 1, 0), (1, o - 1, 0), (0, 0, 1), (2, 2, 2)] + [tuple(rng.integers(0, o, 3)) for _ in range(3)]
@@ -74,6 +90,7 @@ def test_W_matches_oracle(ctx, o, v, naux, seed):
         i, j, k = int(i), int(j), int(k)
         W.fill_(float("nan"))
         ctx.debug_W_triplet(o, v, i, j, k, dp.t2, dp.blocks(), W)
+        assert ctx.get_stats()["kernel"] == TC_KERNEL_TMA          # every v takes the TMA kernel (odd v through padded copies)
         W_ref = oracle.W_triplet(o, v, i, j, k, p.t2, p.vvvo[i], p.vvvo[j], p.vvvo[k], p.ovoo)
         got = W.cpu().numpy()
         scale = np.abs(W_ref).max()
@@ -84,7 +101,7 @@ def test_W_matches_oracle(ctx, o, v, naux, seed):
 # ---- worked closed-form examples (tests/golden/p10_worked_values.txt via the oracle) -----------
 @pytest.mark.parametrize("o,v,naux", [(3, 4, 5), (4, 6, 7), (2, 5, 3), (5, 3, 4)])
 def test_closed_form_examples(ctx, o, v, naux):
-    p = synth.closed_form_problem(o, v, naux)
+    p = harness.closed_form_problem(o, v, naux)
     dp = DevProblem(p)
     n = oracle.triplet_count(o)
     E_ref, S_ref = oracle.triples_energy(p)
@@ -97,18 +114,82 @@ def test_closed_form_examples(ctx, o, v, naux):
 @pytest.mark.parametrize("o,v,naux,seed", [(1, 5, 3, 1), (2, 1, 3, 2), (3, 8, 4, 3), (4, 17, 6, 4), (5, 33, 8, 5), (6, 40, 20, 6)])
 @pytest.mark.parametrize("use_df", [False, True])
 def test_energy_small(ctx, o, v, naux, seed, use_df):
-    p = synth.make_problem(o, v, naux, seed, sigma_B=0.25, blocks=True)
+    p = harness.make_problem(o, v, naux, seed, sigma_B=0.25, blocks=True)
     dp = DevProblem(p)
     n = oracle.triplet_count(o)
     E_ref, S_ref = oracle.triples_energy(p)
-    E, S = run_slice(ctx, dp, 0, n, use_df=use_df)
+    E, S = run_slice(ctx, dp, 0, n, use_df=use_df, expect_kernel=TC_KERNEL_TMA)
+    assert ctx.get_stats()["padded"] == (v % 2)
     tol = REL_TOL * max(np.abs(S_ref).max(), 1e-300)
     assert np.abs(S - S_ref).max() <= tol + (ABS_TOL if np.abs(S_ref).max() < 10 else 0), np.abs(S - S_ref).max()
     assert_energy(E, E_ref)
 
 
+# ---- the paths k_wbuild_tma takes at full size: deferred flush (cps >= 16) with every hole-chunk count,
+#      full range in ONE multi-triplet launch, even v (ragged and not), blocks and DF input --------------------
+DEFERRED_CASES = [(3, 64, 6, 21), (5, 64, 8, 22), (9, 50, 10, 23), (12, 40, 8, 24), (16, 72, 12, 25), (21, 56, 10, 26),
+                  (7, 58, 9, 27)]   # nhc = 1, 2, 3 (ragged v), 3, 4 (ragged), 6, 2 (v mod 16 = 10)
+
+
+@pytest.mark.parametrize("o,v,naux,seed", DEFERRED_CASES)
+@pytest.mark.parametrize("use_df", [False, True])
+def test_energy_deferred_flush_paths(ctx, o, v, naux, seed, use_df):
+    assert chunks_per_step(o, v) >= 16 and v % 2 == 0
+    p = harness.make_problem(o, v, naux, seed, sigma_B=0.25, blocks=True)
+    dp = DevProblem(p)
+    n = oracle.triplet_count(o)
+    E_ref, S_ref = oracle.triples_energy(p)
+    E, S = run_slice(ctx, dp, 0, n, use_df=use_df, expect_kernel=TC_KERNEL_TMA)
+    st = ctx.get_stats()
+    nb16 = (v + 15) // 16
+    assert st["n_work_units"] == n * (nb16 * (nb16 + 1) * (nb16 + 2) // 6) and st["n_blocks"] == 0   # resident regime, one launch
+    assert np.abs(S - S_ref).max() <= REL_TOL * np.abs(S_ref).max(), (np.abs(S - S_ref).max(), np.abs(S_ref).max())
+    assert_energy(E, E_ref)
+
+
+def test_odd_v_takes_the_tma_kernel_and_matches_the_fallback(ctx):
+    """Odd v runs on the TMA kernel through zero-padded copies (row length v + 1); the cp.async kernel, forced through
+    tc_debug_force_kernel, gives the same numbers on the same input."""
+    p = harness.make_problem(6, 37, 9, 33, sigma_B=0.25, blocks=True)
+    dp = DevProblem(p)
+    n = oracle.triplet_count(p.o)
+    E_ref, S_ref = oracle.triples_energy(p)
+    res = {}
+    for use_df in (False, True):
+        res[use_df] = run_slice(ctx, dp, 0, n, use_df=use_df, expect_kernel=TC_KERNEL_TMA)
+        assert ctx.get_stats()["padded"] == 1
+    ctx.force_kernel(TC_KERNEL_CPASYNC)
+    try:
+        res["cp"] = run_slice(ctx, dp, 0, n, expect_kernel=TC_KERNEL_CPASYNC)
+    finally:
+        ctx.force_kernel(TC_KERNEL_AUTO)
+    for E, S in res.values():
+        assert np.abs(S - S_ref).max() <= REL_TOL * np.abs(S_ref).max()
+        assert_energy(E, E_ref)
+
+
+def test_misaligned_caller_pointers_take_the_fallback(ctx):
+    """Caller arrays that are only 8-byte aligned cannot be addressed by TMA: the cp.async kernel runs (and says so)."""
+    p = harness.make_problem(4, 24, 6, 9, sigma_B=0.25, blocks=True)
+    dp = DevProblem(p)
+    n = oracle.triplet_count(p.o)
+    E_ref, S_ref = oracle.triples_energy(p)
+    buf = torch.empty(p.t2.size + 1, dtype=torch.float64, device="cuda")
+    t2_off = buf[1:]                                   # 8 bytes past a 256-byte boundary
+    t2_off.copy_(dp.t2.reshape(-1))
+    assert t2_off.data_ptr() % 16 == 8
+    nb = ctx.workspace_bytes(p.o, p.v, 0)
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    S = torch.empty(n, dtype=torch.float64, device="cuda")
+    E = ctx.triples_energy_slice(p.o, p.v, dp.eps_occ, dp.eps_vir, dp.t1, t2_off, blocks=dp.blocks(), workspace=ws,
+                                 workspace_bytes=nb, first=0, count=n, S_dev=S)
+    assert ctx.get_stats()["kernel"] == TC_KERNEL_CPASYNC
+    assert np.abs(S.cpu().numpy() - S_ref).max() <= REL_TOL * np.abs(S_ref).max()
+    assert_energy(E, E_ref)
+
+
 def test_cfg0_full(ctx):
-    p = synth.make_config("cfg0", blocks=True)
+    p = harness.make_config("cfg0", blocks=True)
     dp = DevProblem(p)
     n = oracle.triplet_count(p.o)
     E_ref, S_ref = oracle.triples_energy(p)
@@ -128,7 +209,7 @@ def test_cfg0_full(ctx):
 
 def test_cfg0_scaled_twin_absolute_bound(ctx):
     """Same shapes as cfg0 with sigma_B reduced so that |E| ~ 1e-3 Eh: the absolute 1e-10 Eh bound binds."""
-    p = synth.make_config("cfg0", blocks=True, sigma_B=0.02)
+    p = harness.make_config("cfg0", blocks=True, sigma_B=0.02)
     dp = DevProblem(p)
     E_ref, S_ref = oracle.triples_energy(p)
     E, S = run_slice(ctx, dp, 0, oracle.triplet_count(p.o))
@@ -137,29 +218,35 @@ def test_cfg0_scaled_twin_absolute_bound(ctx):
     assert np.abs(S - S_ref).max() <= ABS_TOL
 
 
+@pytest.mark.parametrize("dims", [(9, 24, 10, 41), (8, 37, 9, 42), (9, 50, 10, 23)], ids=["v24", "v37-odd", "v50-deferred"])
 @pytest.mark.parametrize("nslots", [3, 4, 7])
-def test_slice_cache_blocked_schedule(ctx, nslots):
+def test_slice_cache_blocked_schedule(ctx, nslots, dims):
     """DF input with a workspace too small for all (vv|v.) slices: the blocked schedule with a slice cache
     (the cfg4 path) must give the same per-triplet S_ijk, on a full range and on a middle slice."""
-    p = synth.make_problem(9, 24, 10, 41, sigma_B=0.25, blocks=True)
+    assert nslots < dims[0]
+    p = harness.make_problem(*dims, sigma_B=0.25, blocks=True)
     dp = DevProblem(p)
     o, v, naux = p.o, p.v, p.naux
     n = oracle.triplet_count(o)
     E_ref, S_ref = oracle.triples_energy(p)
     full = ctx.workspace_bytes(o, v, naux)
-    slice_bytes = (v ** 3 * 8 + 255) // 256 * 256
+    slice_bytes = (v * v * (v + v % 2) * 8 + 255) // 256 * 256
     budget = full - (o - nslots) * slice_bytes
     nb = ctx.workspace_bytes(o, v, naux, budget)
     assert nb <= budget < full
     ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
-    for first, count in ((0, n), (37, 61)):
+    for first, count in ((0, n), (n // 4, n // 3)):
         S = torch.full((count,), float("nan"), dtype=torch.float64, device="cuda")
         E = ctx.triples_energy_slice(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws, workspace_bytes=nb,
                                      first=first, count=count, S_dev=S)
         got = S.cpu().numpy()
         assert np.abs(got - S_ref[first:first + count]).max() <= REL_TOL * np.abs(S_ref).max()
         st = ctx.get_stats()
-        assert st["slices_built"] >= min(o, 3)
+        plan = binding_mod.plan_summary(o, first, count, nslots)
+        assert st["slices_built"] == plan["n_loads"] and st["n_blocks"] == plan["n_blocks"] and st["kernel"] == TC_KERNEL_TMA
+        # a2 runs on the side stream: its interval lies inside the call and starts before the last W-builder ends
+        assert 0.0 <= st["staging_first_ms"] <= st["staging_last_ms"] <= st["ms_total"]
+        assert st["staging_first_ms"] < st["contraction_last_ms"]
     assert_energy(ctx.triples_energy_slice(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws,
                                            workspace_bytes=nb, first=0, count=n), E_ref)
     with pytest.raises(Exception):   # two slots cannot hold the three slices of a triplet
@@ -167,7 +254,7 @@ def test_slice_cache_blocked_schedule(ctx, nslots):
 
 
 def test_host_entry_point(ctx):
-    p = synth.make_problem(4, 21, 9, 21, sigma_B=0.25, blocks=True)
+    p = harness.make_problem(4, 21, 9, 21, sigma_B=0.25, blocks=True)
     E_ref, _ = oracle.triples_energy(p)
     E, nbytes = ctx.triples_energy_host(p.o, p.v, p.naux, p.eps_occ, p.eps_vir, p.t1, p.t2, p.Boo, p.Bov, p.Bvv)
     assert_energy(E, E_ref)
@@ -175,7 +262,7 @@ def test_host_entry_point(ctx):
 
 
 def test_build_blocks_matches_oracle(ctx):
-    p = synth.make_problem(4, 21, 9, 31, blocks=False)
+    p = harness.make_problem(4, 21, 9, 31, blocks=False)
     dp = DevProblem(p)
     o, v, naux = p.o, p.v, p.naux
     vvvo = torch.empty((o, v, v, v), dtype=torch.float64, device="cuda")
@@ -190,8 +277,22 @@ def test_build_blocks_matches_oracle(ctx):
     assert np.abs(ovov.cpu().numpy() - oracle.build_ovov(o, v, naux, p.Bov)).max() <= 1e-14 * naux
 
 
-def test_deterministic(ctx):
-    p = synth.make_problem(5, 33, 8, 5, sigma_B=0.25, blocks=True)
+def test_deterministic_tma_kernel(ctx):
+    """Bit-reproducibility of the TMA kernel on a deferred-flush size (cps >= 16), full range, four runs: the flush has
+    no CTA barrier and rests on a ring-ordering argument -- a race would show up here first."""
+    p = harness.make_problem(9, 50, 10, 23, sigma_B=0.25, blocks=True)
+    assert chunks_per_step(p.o, p.v) >= 16
+    dp = DevProblem(p)
+    n = oracle.triplet_count(p.o)
+    runs = [run_slice(ctx, dp, 0, n, use_df=(r % 2 == 1), expect_kernel=TC_KERNEL_TMA) for r in range(6)]
+    for r in (2, 4):
+        assert runs[r][0] == runs[0][0] and (runs[r][1] == runs[0][1]).all()
+    for r in (3, 5):
+        assert runs[r][0] == runs[1][0] and (runs[r][1] == runs[1][1]).all()
+
+
+def test_deterministic_odd_v(ctx):
+    p = harness.make_problem(5, 33, 8, 5, sigma_B=0.25, blocks=True)
     dp = DevProblem(p)
     n = oracle.triplet_count(p.o)
     E1, S1 = run_slice(ctx, dp, 0, n)
@@ -201,14 +302,21 @@ def test_deterministic(ctx):
 
 def test_argument_errors(ctx):
     from paper_2512_01055_b200.binding import TcError
-    p = synth.make_problem(3, 8, 4, 3, blocks=True)
+    p = harness.make_problem(3, 8, 4, 3, blocks=True)
     dp = DevProblem(p)
     ws = torch.empty(1 << 20, dtype=torch.uint8, device="cuda")
     with pytest.raises(TcError):   # both blocks and df
         ctx.triples_energy(p.o, p.v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, blocks=dp.blocks(), df=dp.df(), workspace=ws,
                            workspace_bytes=ws.numel())
-    with pytest.raises(TcError):   # workspace too small
+    with pytest.raises(TcError) as e:   # workspace too small
         ctx.triples_energy(p.o, p.v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, blocks=dp.blocks(), workspace=ws, workspace_bytes=16)
+    assert e.value.status == 3
+    with pytest.raises(TcError) as e:   # workspace_bytes = 0 is "too small", never "unbounded" (blocks and DF input)
+        ctx.triples_energy(p.o, p.v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, blocks=dp.blocks(), workspace=ws, workspace_bytes=0)
+    assert e.value.status == 3
+    with pytest.raises(TcError) as e:
+        ctx.triples_energy(p.o, p.v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws, workspace_bytes=0)
+    assert e.value.status == 3
     with pytest.raises(TcError):   # range outside
         ctx.triples_energy_slice(p.o, p.v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, blocks=dp.blocks(), workspace=ws,
                                  workspace_bytes=ws.numel(), first=5, count=100)
@@ -217,19 +325,73 @@ def test_argument_errors(ctx):
                            workspace_bytes=ws.numel())
 
 
-def test_empty_range_and_fallback_kernel_on_even_v(ctx, monkeypatch):
-    """count = 0 is a valid (empty) range; the cp.async fallback kernel (used for odd v) gives the same numbers as the
-    TMA kernel on an even-v problem (TC_FORCE_CPASYNC is a testing aid of the library)."""
-    p = synth.make_problem(4, 24, 6, 9, sigma_B=0.25, blocks=True)
+def test_empty_range_and_fallback_kernel_on_even_v(ctx):
+    """count = 0 is a valid (empty) range; the cp.async fallback kernel gives the same numbers as the TMA kernel on an
+    even-v problem (tc_debug_force_kernel is a validation aid of the library)."""
+    p = harness.make_problem(4, 24, 6, 9, sigma_B=0.25, blocks=True)
     dp = DevProblem(p)
     n = oracle.triplet_count(p.o)
     E0, _ = run_slice(ctx, dp, 3, 0)
     assert E0 == 0.0
     E_ref, S_ref = oracle.triples_energy(p)
-    E_tma, S_tma = run_slice(ctx, dp, 0, n)
-    monkeypatch.setenv("TC_FORCE_CPASYNC", "1")
-    E_cp, S_cp = run_slice(ctx, dp, 0, n)
-    monkeypatch.delenv("TC_FORCE_CPASYNC")
+    E_tma, S_tma = run_slice(ctx, dp, 0, n, expect_kernel=TC_KERNEL_TMA)
+    ctx.force_kernel(TC_KERNEL_CPASYNC)
+    try:
+        E_cp, S_cp = run_slice(ctx, dp, 0, n, expect_kernel=TC_KERNEL_CPASYNC)
+    finally:
+        ctx.force_kernel(TC_KERNEL_AUTO)
     for E, S in ((E_tma, S_tma), (E_cp, S_cp)):
         assert np.abs(S - S_ref).max() <= REL_TOL * np.abs(S_ref).max()
         assert_energy(E, E_ref)
+
+
+# ---- NEXT-3: host-resident amplitudes streamed through a device ring of rows (PAPER.md:57, 69) -----------------
+@pytest.mark.parametrize("o,v,naux,seed,nslots", [(9, 24, 10, 41, 4), (9, 24, 10, 41, 9), (7, 37, 9, 42, 5), (12, 40, 8, 24, 6)])
+def test_streamed_t2_from_host(ctx, o, v, naux, seed, nslots):
+    p = harness.make_problem(o, v, naux, seed, sigma_B=0.25, blocks=True)
+    dp = DevProblem(p)
+    n = oracle.triplet_count(o)
+    E_ref, S_ref = oracle.triples_energy(p)
+    t2_host = torch.from_numpy(np.ascontiguousarray(p.t2)).pin_memory()
+    full = ctx.workspace_bytes_streamed(o, v, naux)
+    ldv = v + (v % 2)
+    per_slot = (v * v * ldv * 8 + 255) // 256 * 256 + (o * v * ldv * 8 + 255) // 256 * 256
+    budget = full - (o - nslots) * per_slot
+    nb = ctx.workspace_bytes_streamed(o, v, naux, budget)
+    assert nb <= budget <= full
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    for first, count in ((0, n), (n // 3, n // 2)):
+        S = torch.full((count,), float("nan"), dtype=torch.float64, device="cuda")
+        E = ctx.triples_energy_streamed(o, v, dp.eps_occ, dp.eps_vir, dp.t1, t2_host, df=dp.df(), workspace=ws,
+                                        workspace_bytes=nb, first=first, count=count, S_dev=S)
+        st = ctx.get_stats()
+        plan = binding_mod.plan_summary(o, first, count, nslots)
+        assert st["t2_rows_copied"] == plan["n_loads"] == st["slices_built"] and st["kernel"] == TC_KERNEL_TMA
+        assert st["bytes_h2d"] == plan["n_loads"] * o * v * v * 8
+        assert np.abs(S.cpu().numpy() - S_ref[first:first + count]).max() <= REL_TOL * np.abs(S_ref).max()
+        if first == 0:
+            assert_energy(E, E_ref)
+    with pytest.raises(binding_mod.TcError):   # a device pointer where the host array is expected
+        ctx.triples_energy_streamed(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws, workspace_bytes=nb,
+                                    first=0, count=n)
+
+
+# ---- NEXT-1: triplet ranges per rank behind the boundary (PAPER.md:63, 77), all ranks' ranges on this one GPU --------
+@pytest.mark.parametrize("world", [2, 3])
+def test_partitioned_ranges_sum_to_the_full_energy(ctx, world):
+    p = harness.make_config("cfg0", blocks=True)
+    dp = DevProblem(p)
+    n = oracle.triplet_count(p.o)
+    E_ref, S_ref = oracle.triples_energy(p)
+    E_full, _ = run_slice(ctx, dp, 0, n, use_df=True)
+    parts, covered = [], 0
+    for rank in range(world):
+        first, count = binding_mod.triplet_partition(p.o, world, rank)
+        assert first == covered
+        covered += count
+        E_r, S_r = run_slice(ctx, dp, first, count, use_df=True)
+        assert np.abs(S_r - S_ref[first:first + count]).max() <= REL_TOL * np.abs(S_ref).max()
+        parts.append(E_r)
+    assert covered == n
+    assert_energy(sum(parts), E_ref)
+    assert abs(sum(parts) - E_full) <= 1e-13 * abs(E_full)

@@ -11,6 +11,7 @@ import os
 import numpy as np
 import pytest
 
+import harness
 import oracle
 from paper_2512_01055_b200 import synth
 
@@ -143,7 +144,7 @@ def _golden_rows():
 @pytest.mark.parametrize("row", _golden_rows(), ids=lambda r: f"{r[0]}-{r[1]}{r[2]}{r[3]}-{''.join(r[4])}")
 def test_p10_worked_values(row):
     kind, o, v, naux, ix, val = row
-    p = synth.closed_form_problem(o, v, naux, t1_zero=(kind == "E_t1zero"))
+    p = harness.closed_form_problem(o, v, naux, t1_zero=(kind == "E_t1zero"))
     ii = [None if s == "-" else int(s) for s in ix]
     if kind in ("E", "E_t1zero"):
         got, _ = oracle.triples_energy(p)
@@ -176,7 +177,7 @@ def test_p10_worked_values(row):
 # ----------------------------------------------------------------------------
 @pytest.fixture(scope="module")
 def small():
-    return synth.make_problem(4, 6, 9, seed=11, blocks=True)
+    return harness.make_problem(4, 6, 9, seed=11, blocks=True)
 
 
 def test_p1_zero_amplitudes(small):
@@ -224,7 +225,7 @@ def _relabel(p, perm_o, perm_v):
                       np.ascontiguousarray(p.Boo[:, perm_o][:, :, perm_o]),
                       np.ascontiguousarray(p.Bov[:, perm_o][:, :, perm_v]),
                       np.ascontiguousarray(p.Bvv[:, perm_v][:, :, perm_v]))
-    return synth.materialise_blocks(q)
+    return oracle.blocks.materialise_blocks(q)
 
 
 def test_p4_relabelling_invariance(small):
@@ -260,13 +261,13 @@ def test_p6_negative_semidefinite_when_t1_zero(small):
 
 
 def test_p7_degenerate_sizes():
-    p = synth.make_problem(1, 5, 4, seed=3, blocks=True)
+    p = harness.make_problem(1, 5, 4, seed=3, blocks=True)
     E, S = oracle.triples_energy(p)
     assert abs(E) < 1e-18
-    p = synth.make_problem(3, 1, 4, seed=3, blocks=True)
+    p = harness.make_problem(3, 1, 4, seed=3, blocks=True)
     E, S = oracle.triples_energy(p)
     assert abs(E) < 1e-18 and np.all(np.abs(S) < 1e-18)
-    p = synth.make_problem(3, 4, 4, seed=3, blocks=True)
+    p = harness.make_problem(3, 4, 4, seed=3, blocks=True)
     _, S = oracle.triples_energy(p)
     for i in range(3):
         assert abs(S[IDX(i, i, i)]) < 1e-18 * max(1.0, np.abs(S).max()) + 1e-20
@@ -277,7 +278,7 @@ def test_p7_degenerate_sizes():
 # ----------------------------------------------------------------------------
 @pytest.mark.parametrize("dims", [(3, 4, 5), (2, 5, 3), (4, 3, 6)])
 def test_p8_paper_printed_form(dims):
-    p = synth.make_problem(*dims, seed=21, sigma_B=0.3, sigma_t1=0.05, blocks=True)
+    p = harness.make_problem(*dims, seed=21, sigma_B=0.3, sigma_t1=0.05, blocks=True)
     E, _ = oracle.triples_energy(p)
     Ep, W6 = paper_form_energy(p)
     assert E == pytest.approx(Ep, rel=1e-12)
@@ -290,23 +291,27 @@ def test_p8_paper_printed_form(dims):
 
 @pytest.mark.parametrize("dims", [(2, 3, 4), (3, 3, 5), (2, 4, 3)])
 def test_p9_spin_orbital_textbook_formula(dims):
-    p = synth.make_problem(*dims, seed=31, sigma_B=0.3, sigma_t1=0.05, blocks=True)
+    p = harness.make_problem(*dims, seed=31, sigma_B=0.3, sigma_t1=0.05, blocks=True)
     E, _ = oracle.triples_energy(p)
     Es = spin_orbital_energy(p)
     assert E == pytest.approx(Es, rel=1e-11)
 
 
-def test_p9_closed_form_example():
-    p = synth.closed_form_problem(3, 4, 5)
-    assert spin_orbital_energy(p) == pytest.approx(-0.0311103618453645, rel=1e-11)
-    assert paper_form_energy(p)[0] == pytest.approx(-0.0311103618453645, rel=1e-11)
+@pytest.mark.parametrize("o,v,naux", [(3, 4, 5), (4, 6, 7), (2, 5, 3), (5, 3, 4)])
+def test_p9_closed_form_example(o, v, naux):
+    """Every E in tests/golden/p10_worked_values.txt is re-derived here by two formulas that share nothing with the
+    oracle (the spin-orbital textbook formula and the paper's own printed form), so the file stands on its own."""
+    golden = {(r[1], r[2], r[3]): r[5] for r in _golden_rows() if r[0] == "E"}
+    p = harness.closed_form_problem(o, v, naux)
+    assert spin_orbital_energy(p) == pytest.approx(golden[(o, v, naux)], rel=1e-11)
+    assert paper_form_energy(p)[0] == pytest.approx(golden[(o, v, naux)], rel=1e-11)
 
 
 # ----------------------------------------------------------------------------
 # DF builders against a library contraction, triplet index, slices entry
 # ----------------------------------------------------------------------------
 def test_df_builders_against_einsum():
-    p = synth.make_problem(3, 5, 7, seed=2, blocks=True)
+    p = harness.make_problem(3, 5, 7, seed=2, blocks=True)
     o, v, naux = p.o, p.v, p.naux
     eri = full_eri(p)
     O, V = slice(0, o), slice(o, o + v)
@@ -321,6 +326,28 @@ def test_df_builders_against_einsum():
     ovov = oracle.build_ovov(o, v, naux, p.Bov)
     np.testing.assert_allclose(ovov, eri[O, V, O, V].transpose(0, 2, 1, 3), rtol=1e-13, atol=1e-15)  # (jb|kc)->[j][k][b][c]
     np.testing.assert_allclose(p.ovov, ovov, rtol=1e-13, atol=1e-15)
+
+
+def test_pair_panels_and_amplitude_rows():
+    """The restricted builders the large-size goldens use (only the panels / amplitude rows a few triplets touch)
+    agree with the full ones."""
+    p = harness.make_problem(5, 6, 7, seed=4, blocks=True)
+    occ = [4, 1, 2]
+    ovoo, ovov = oracle.blocks.ovoo_pairs(p, occ), oracle.blocks.ovov_pairs(p, occ)
+    for x in occ:
+        for y in occ:
+            np.testing.assert_allclose(ovoo[x, y], p.ovoo[x, y], rtol=1e-13, atol=1e-16)
+            np.testing.assert_allclose(ovov[x, y], p.ovov[x, y], rtol=1e-13, atol=1e-16)
+    rows = synth.mp2_amplitude_rows(p.Bov, p.eps_occ, p.eps_vir, occ)
+    for x in occ:
+        np.testing.assert_allclose(rows[x], p.t2[x], rtol=1e-13, atol=1e-18)
+    assert not rows[0].any() and not rows[3].any()
+    # the oracle reads t2 only through rows whose first index is one of i, j, k
+    idx = IDX(4, 2, 1)
+    q = synth.Problem(p.o, p.v, p.naux, p.eps_occ, p.eps_vir, p.t1, rows, p.Boo, p.Bov, p.Bvv, None, ovoo, ovov)
+    _, S_rows = oracle.triples_energy_slices(q, {x: p.vvvo[x] for x in occ}, idx, 1)
+    _, S_full = oracle.triples_energy(p, idx, 1)
+    assert S_rows[0] == pytest.approx(S_full[0], rel=1e-12)
 
 
 def test_triplet_index_is_a_bijection():

@@ -1,5 +1,5 @@
 """Host-side logic of the N>1 path (bench.py --gpus N): the linear triplet index is cut into N contiguous
-ranges, every rank reduces its own range and the only exchange is one all-reduce of the FP64 partial
+ranges (tc_triplet_partition), every rank reduces its own range and the only exchange is one all-reduce of the FP64 partial
 energy (paper: independent tile batches per GPU, partial energies summed).
 Run on CPU with the gloo backend, world_size 2 and 3; the per-range partial energies come from the CPU oracle
 (the per-range CUDA call is covered by test_gpu_parity.py::test_cfg0_full)."""
@@ -18,15 +18,16 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def _worker(rank, world, port, q):
     sys.path.insert(0, ROOT)
-    import bench
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import harness
     import oracle
-    from paper_2512_01055_b200 import synth
+    from paper_2512_01055_b200 import binding
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
-    p = synth.make_problem(5, 6, 7, seed=3, sigma_B=0.3, blocks=True)
+    p = harness.make_problem(5, 6, 7, seed=3, sigma_B=0.3, blocks=True)
     n = oracle.triplet_count(p.o)
-    first, count = bench.partition(n, world, rank)
+    first, count = binding.triplet_partition(p.o, world, rank)     # the library's own partition (C-ABI, host only)
     E_part, _ = oracle.triples_energy(p, first, count) if count else (0.0, None)
     t = torch.tensor([E_part, float(count)], dtype=torch.float64)
     dist.all_reduce(t, op=dist.ReduceOp.SUM)
@@ -54,18 +55,3 @@ def test_partition_and_allreduce(world):
     assert n_sum == n                       # the ranges tile [0, N_trip)
     assert abs(E_sum - E_full) <= 1e-12 * abs(E_full)
     assert tmax == world                    # max over ranks
-
-
-def test_partition_tiles_the_index_range():
-    sys.path.insert(0, ROOT)
-    import bench
-    for n in (1, 7, 120, 1540):
-        for world in (1, 2, 3, 4, 8):
-            at = 0
-            sizes = []
-            for r in range(world):
-                first, count = bench.partition(n, world, r)
-                assert first == at and count >= 0
-                at += count
-                sizes.append(count)
-            assert at == n and max(sizes) - min(sizes) <= 1
