@@ -346,6 +346,9 @@ tc_status run_energy(tc_ctx* ctx, int o, int v, const double* eps_occ, const dou
             double* h_w = (double*)(h_recs + nrec);
             int* h_dest = (int*)(h_w + nrec);
             memcpy(h_recs, plan.recs.data(), nrec * sizeof(tc_trip_rec));
+            if (mode != MODE_STREAMED)   // t2 is resident as a whole: its rows are addressed by occupied index, not by slot
+                for (size_t r = 0; r < nrec; r++)
+                    for (int q = 0; q < 3; q++) h_recs[r].t[q] = h_recs[r].occ[q];
             memcpy(h_dest, plan.dest.data(), nrec * sizeof(int));
             for (size_t r = 0; r < nrec; r++) {   // w[dest] = 2 - d_ij - d_jk (eq. (1))
                 const tc_trip_rec& rec = plan.recs[r];
