@@ -189,7 +189,7 @@ def measure_slice(ctx, torch, synth, name, first, count, dmma_peak, reps=2):
     out = {"workload": f"{name}: o={o}, v={v}, naux={naux}, seed {seed}, triplets [{first},{first + count})", "tflops": tf,
            "frac_of_dmma_peak": tf / dmma_peak, "kernel_tflops": tfk, "kernel_frac": tfk / dmma_peak, "ms_total": best["ms_total"],
            "ms_kernels": best["ms_kernels"], "ms_staging": best["ms_staging"], "slices_built": best["slices_built"],
-           "n_blocks": best["n_blocks"], "kernel": {1: "k_wbuild_tma", 2: "k_wbuild (cp.async)"}.get(best["kernel"]),
+           "n_blocks": best["n_blocks"], "kernel": {1: "k_wbuild_tma"}.get(best["kernel"]),
            "padded": best["padded"], "staging_interval_ms": [best["staging_first_ms"], best["staging_last_ms"]],
            "contraction_interval_ms": [best["contraction_first_ms"], best["contraction_last_ms"]],
            "E_partial": E, "input_generation_s": t_gen, "clocks": clocks}
@@ -298,7 +298,8 @@ def run_ours(args):
         try:
             full_s = ctx.workspace_bytes_streamed(o, v, naux)
             ldv = v + (v % 2)
-            per_slot = (v * v * ldv * 8 + 255) // 256 * 256 + (o * v * ldv * 8 + 255) // 256 * 256
+            nb16, nkq = (v + 15) // 16, (v + 3) // 4
+            per_slot = (nb16 * nb16 * nkq * 8192 + 255) // 256 * 256 + (o * v * ldv * 8 + 255) // 256 * 256
             nb_s = ctx.workspace_bytes_streamed(o, v, naux, full_s - (o - max(3, o // 2)) * per_slot)
             ws_s = ws[:nb_s] if nb_s <= nb else torch.empty(nb_s, dtype=torch.uint8, device="cuda")
             best = None

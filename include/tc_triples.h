@@ -140,7 +140,9 @@ tc_status tc_build_blocks(tc_ctx* ctx, int o, int v, const tc_df_factors* df,
 
 /* E(T) over all triplets.  Exactly one of `blocks` / `df` is non-NULL.
  *   eps_occ[o], eps_vir[v], t1[i][a], t2[i][j][a][b] (= t_ij^ab; precondition
- *   t_ij^ab == t_ji^ba): device.  E_out: host.  */
+ *   t_ij^ab == t_ji^ba): device.  t2 must be 16-byte aligned (it is a TMA operand; CUDA allocators
+ *   return at least 256-byte alignment), else TC_ERR_INVALID_ARG.  Any o, v >= 1: odd v runs on the
+ *   same kernel through a zero-padded copy of t2 in the workspace.  E_out: host.  */
 tc_status tc_triples_energy(tc_ctx* ctx, int o, int v,
                             const double* eps_occ, const double* eps_vir,
                             const double* t1, const double* t2,
@@ -193,14 +195,7 @@ tc_status tc_triples_energy_host(tc_ctx* ctx, int o, int v, int naux,
 tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j, int k,
                              const double* t2, const tc_int_blocks* blocks,
                              double* W_dev, void* stream);
-/* Debug/validation: which W-builder kernel the next calls on ctx use.  TC_KERNEL_AUTO (default): the
- * TMA/mbarrier kernel whenever the operands can be addressed by TMA (always, except for caller pointers
- * that are not 16-byte aligned), else the cp.async kernel.  TC_KERNEL_CPASYNC forces the latter so the
- * tests can check it on any input. */
-#define TC_KERNEL_AUTO    0
-#define TC_KERNEL_TMA     1
-#define TC_KERNEL_CPASYNC 2
-tc_status tc_debug_force_kernel(tc_ctx* ctx, int which);
+#define TC_KERNEL_TMA 1 /* tc_stats.kernel: the TMA/mbarrier/TMEM W-builder (the only one there is) */
 
 /* ---- statistics of the last energy call ----------------------------------------- */
 
@@ -213,8 +208,8 @@ typedef struct {
     double    ms_contraction;    /* device time of the fused W-builder kernels           */
     double    ms_staging;        /* device time of DF->block assembly (0 with blocks)    */
     long long slices_built;      /* (vv|v.) slices assembled from DF during the call     */
-    int       kernel;            /* W-builder that ran: TC_KERNEL_TMA or TC_KERNEL_CPASYNC */
-    int       padded;            /* 1: odd v, operands used through zero-padded copies (row length v+1) */
+    int       kernel;            /* W-builder that ran: TC_KERNEL_TMA (0 if the range was empty) */
+    int       padded;            /* 1: odd v, t2 used through a zero-padded copy (row length v+1) */
     long long n_blocks;          /* blocked schedule: W-builder launches (0 = everything resident) */
     long long t2_rows_copied;    /* streamed call: amplitude rows copied host->device    */
     double    bytes_h2d;         /* streamed call: bytes copied host->device             */

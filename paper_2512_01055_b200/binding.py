@@ -15,10 +15,10 @@ from typing import Optional, Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libtc_triples.so")
+LIB_PATH = os.environ.get("TC_TRIPLES_LIB") or os.path.join(_HERE, "libtc_triples.so")   # override: a differently built copy
 
 TC_OK = 0
-TC_KERNEL_AUTO, TC_KERNEL_TMA, TC_KERNEL_CPASYNC = 0, 1, 2
+TC_KERNEL_TMA = 1
 _STATUS = {0: "TC_OK", 1: "TC_ERR_INVALID_ARG", 2: "TC_ERR_UNSUPPORTED_DEVICE", 3: "TC_ERR_WORKSPACE_TOO_SMALL",
            4: "TC_ERR_CUDA", 5: "TC_ERR_INTERNAL"}
 
@@ -56,7 +56,7 @@ EXPORTS = [
     "tc_triplet_count", "tc_triplet_decode", "tc_triplet_index", "tc_triplet_partition",
     "tc_workspace_bytes", "tc_workspace_bytes_streamed", "tc_plan_summary", "tc_plan_dump", "tc_build_blocks",
     "tc_triples_energy", "tc_triples_energy_slice", "tc_triples_energy_streamed", "tc_triples_energy_host",
-    "tc_debug_W_triplet", "tc_debug_force_kernel",
+    "tc_debug_W_triplet",
     "tc_get_stats", "tc_bench_dmma_peak", "tc_bench_dfma_peak", "tc_bench_copy_bw", "tc_bench_ring_peak",
 ]
 
@@ -91,7 +91,6 @@ def lib() -> ctypes.CDLL:
     L.tc_plan_summary.argtypes = [_i, _ll, _ll, _i, _P(_ll), _P(_ll), _P(_i), _P(_i), _P(_i)]
     L.tc_plan_dump.argtypes = [_i, _ll, _ll, _i, _vp, _vp, _ll]
     L.tc_triples_energy_streamed.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_DfFactors), _vp, _sz, _vp, _ll, _ll, _vp, _P(_d)]
-    L.tc_debug_force_kernel.argtypes = [_vp, _i]
     L.tc_bench_ring_peak.argtypes = [_vp, _i, _d, _vp, _sz, _P(_d)]
     L.tc_build_blocks.argtypes = [_vp, _i, _i, _P(_DfFactors), _i, _i, _vp, _vp, _vp, _vp]
     L.tc_triples_energy.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_IntBlocks), _P(_DfFactors), _vp, _sz, _vp, _P(_d)]
@@ -224,9 +223,6 @@ class Context:
     def debug_W_triplet(self, o, v, i, j, k, t2, blocks: Sequence, W_dev, stream=None):
         b = _IntBlocks(*[_ptr(x) for x in blocks])
         self._check(lib().tc_debug_W_triplet(self._h, o, v, i, j, k, _ptr(t2), ctypes.byref(b), _ptr(W_dev), _stream(stream)))
-
-    def force_kernel(self, which: int = TC_KERNEL_AUTO):
-        self._check(lib().tc_debug_force_kernel(self._h, which))
 
     def get_stats(self) -> dict:
         s = TcStats()

@@ -33,7 +33,6 @@ struct tc_ctx {
     size_t host_slab_bytes;
     void* plan_host;               // pinned host staging of the blocked schedule's tables (grow-only)
     size_t plan_host_bytes;
-    int force_kernel;              // tc_debug_force_kernel: 0 auto, 2 cp.async kernel (validation of the fallback)
     tc_stats stats;
     char err[512];
 };
@@ -89,6 +88,15 @@ __device__ __forceinline__ void cp_async_wait() {
 cudaError_t tc_launch_df_gemm(const double* A, size_t lda, const double* B, size_t ldb, int M, int N, int K,
                               int R2, long long sr1, long long sr2, int C2, long long sc1, long long sc2,
                               double* C, cudaStream_t stream);
+// a2 for the W-builder: slices x0 .. x0+nx-1, I_x[d][b][c] = (bd|cx) = sum_Q Bvv[Q][d][b] Bov[Q][x][c], written in the tiled
+// layout (slice x at dst + (x - x0) * slice_stride; the zero padding is NOT written: the caller clears the slots once).
+cudaError_t tc_launch_df_slices_tiled(const double* Bvv, const double* Bov, int o, int v, int naux, int x0, int nx,
+                                      double* dst, size_t slice_stride, cudaStream_t stream);
+// the same layout from a materialised array src[k][b][c] (K rows k, row length ld >= v): a slice of the caller's (vv|vo)
+// block (K = v) or an amplitude row t2[y] (K = o); writes the padding too
+cudaError_t tc_launch_tile_slice(const double* src, int K, int v, size_t ld, double* dst, cudaStream_t stream);
+// (ov|oo)^T[z][x][m][ldo] from the caller's block ovoo[z][x][l][m] (blocks input); the pad column is zeroed
+cudaError_t tc_launch_transpose_ovoo(const double* ovoo, int o, int v, int ldo, double* dst, cudaStream_t stream);
 
 // a3-a6: fused W-builder + epilogue over a list of triplets (tc_wbuild_tma.cu, tc_wbuild.cu).
 // One record per triplet.  The slots say where the per-occupied-index operands of the triplet live: slice slot s[p]
@@ -106,42 +114,40 @@ static_assert(sizeof(tc_trip_rec) == 48, "tc_trip_rec is read as three int4");
 
 struct tc_wbuild_args {
     int o, v;
-    int ldv;                         // row length (doubles) of t2, ovoo and the slices: v, or v + 1 for odd v (padded copies)
+    int ldv;                         // row length (doubles) of t2: v, or v + 1 for odd v (zero-padded copy)
+    int ldo;                         // row length of (ov|oo)^T: o rounded up to even
     const double* eps_occ;
     const double* eps_vir;
     const double* t1;
     const double* t2;                // [tslot][y][a][ldv], amplitude rows t2_row_stride doubles apart
     size_t t2_row_stride;
-    const double* slices;            // slot s at slices + s * slice_stride, laid out [d][b][ldv]
+    const double* slices;            // slot s at slices + s * slice_stride, in the W-builder's tiled layout
+                                     // [n1 tile][n2 tile][K chunk][z][n1 16][k 4][n2 8], zero padded (tc_wbuild_slice_doubles)
     size_t slice_stride;             // doubles
-    const double* ovoo;              // [z][x][l][ldv]
-    const double* ovov;              // [j][k][b][c] (unpadded; read by the epilogue only)
+    const double* ovooT;             // [z][x][m][ldo] = (l z | x m): the (ov|oo) block with the contracted index fastest
+    const double* ovov;              // [j][k][b][c] (natural layout; read by the epilogue only)
     const tc_trip_rec* recs;         // device array [n_trip]
     int n_trip;
     double* partial;                 // device [n_trip][n_orbits] per-unit partial sums
     int n_orbits;
     double* W_debug;                 // optional v^3 output of W for n_trip == 1
 };
-// TMA descriptors of the four operand streams of the main-path kernel (tc_wbuild_tma.cu).
+// TMA descriptors of the tensor-box operand streams (tc_wbuild_tma.cu); the slices are read with plain bulk copies.
 struct tc_wbuild_maps {
-    CUtensorMap I;     // (vv|v.) slices   [slot][d][b][c]
-    CUtensorMap T2h;   // t2 as hole B     [tslot][l][n1][n2]
-    CUtensorMap T2p;   // t2 as particle A [tslot][y][m][d]
-    CUtensorMap Ovoo;  // (ov|oo) hole A   [z][x][l][m]
-    bool valid;        // false: a base pointer or stride is not 16-byte aligned -> cp.async fallback kernel
+    CUtensorMap T2h;    // t2 as hole B        [tslot][l][n1][n2]
+    CUtensorMap T2p;    // t2 as particle A    [tslot][y][m][d]
+    CUtensorMap OvooT;  // (ov|oo)^T as hole A [z][x][m][l]
+    bool valid;
 };
-// nslots slices and n_tslots amplitude rows behind a.slices / a.t2.
-cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, int nslots, int n_tslots, tc_wbuild_maps* out);
+// n_tslots amplitude rows behind a.t2.
+cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, int n_tslots, tc_wbuild_maps* out);
 int tc_wbuild_tile();                                  // virtual tile edge T
 int tc_wbuild_num_orbits(int v);                       // nb(nb+1)(nb+2)/6
-// maps == NULL or !maps->valid: cp.async kernel (any alignment); else the TMA/mbarrier kernel.  Returns which ran
-// through *kernel_out (TC_KERNEL_TMA / TC_KERNEL_CPASYNC).
+size_t tc_wbuild_slice_doubles(int v);                 // doubles of one slice in the tiled layout
 cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const tc_wbuild_maps* maps,
-                             const int4* orbits /*device [n_orbits]: (A,B,C,0), A>=B>=C*/, cudaStream_t stream, int* kernel_out);
-cudaError_t tc_launch_wbuild_cpasync(const tc_wbuild_args& a, const int4* orbits, cudaStream_t stream);
+                             const int4* orbits /*device [n_orbits]: (A,B,C,0), A>=B>=C*/, cudaStream_t stream);
 // per-device kernel attributes (opt-in shared memory); called by tc_create with the device current
 cudaError_t tc_wbuild_configure();
-cudaError_t tc_wbuild_cpasync_configure();
 cudaError_t tc_stager_configure();
 cudaError_t tc_microbench_configure();
 

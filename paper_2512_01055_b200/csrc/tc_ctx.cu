@@ -52,7 +52,7 @@ extern "C" tc_status tc_create(tc_ctx** out, int device) {
     for (int n = 0; n < 6; n++) ok = ok && cudaEventCreate(timed[n]) == cudaSuccess;
     ok = ok && cudaMallocHost(&ctx->pinned, 64 * sizeof(double)) == cudaSuccess;
     // opt-in shared memory of the kernels: a per-device attribute, set here for this context's device
-    ok = ok && tc_wbuild_configure() == cudaSuccess && tc_wbuild_cpasync_configure() == cudaSuccess &&
+    ok = ok && tc_wbuild_configure() == cudaSuccess &&
          tc_stager_configure() == cudaSuccess && tc_microbench_configure() == cudaSuccess;
     if (!ok) {
         tc_destroy(ctx);

@@ -21,15 +21,16 @@ enum Mode { MODE_BLOCKS = 0, MODE_DF = 1, MODE_STREAMED = 2 };
 // (pre-allocate and reuse; no device allocation inside the call).
 struct Layout {
     size_t off_orbits, off_recs, off_dest, off_w, off_S, off_partial, off_E;
-    size_t off_t2;      // padded copy of t2 (odd v, resident t2) or the amplitude-row slots (streamed)
-    size_t off_ovoo;    // (ov|oo): assembled from DF, or the padded copy of the caller's block (odd v)
+    size_t off_t2;      // zero-padded copy of t2 (odd v, resident t2) or the amplitude-row slots (streamed)
+    size_t off_ovooT;   // (ov|oo)^T [z][x][m][ldo]: assembled from DF, or transposed from the caller's block
     size_t off_ovov;    // (ov|ov) assembled from DF
-    size_t off_vvvo;    // slice slots: assembled from DF, or the padded copy of the caller's block (odd v)
+    size_t off_vvvo;    // slice slots in the W-builder's tiled layout: assembled from DF, or re-tiled from the caller's block
     size_t total;
     int n_orbits;
     int batch;          // triplets per W-builder launch (resident regime)
     int n_slots;        // resident (vv|v.) slices; < o: blocked schedule
-    int ldv;            // row length of the TMA-addressed operands: v, or v + 1 when v is odd
+    int ldv;            // row length of the TMA-addressed t2: v, or v + 1 when v is odd
+    int ldo;            // row length of (ov|oo)^T: o rounded up to even
     size_t slice_stride, t2row_stride;   // doubles
 };
 
@@ -45,6 +46,7 @@ bool make_layout(int o, int v, int naux, Mode mode, bool bounded, size_t budget,
     if (batch * L->n_orbits > 0x7fffffffLL) batch = 0x7fffffffLL / L->n_orbits;
     L->batch = (int)batch;
     L->ldv = v + (v & 1);
+    L->ldo = o + (o & 1);
     const bool pad = L->ldv != v;
     const size_t O = o, V = v, LD = L->ldv;
     size_t off = 0;
@@ -60,19 +62,15 @@ bool make_layout(int o, int v, int naux, Mode mode, bool bounded, size_t budget,
     L->off_S = take(sizeof(double) * (size_t)ntrip);
     L->off_partial = take(sizeof(double) * (size_t)L->batch * L->n_orbits);
     L->off_E = take(sizeof(double) * 8);
-    L->off_t2 = L->off_ovoo = L->off_ovov = L->off_vvvo = 0;
-    L->slice_stride = align_up(sizeof(double) * V * V * LD) / sizeof(double);
+    L->off_t2 = L->off_ovov = 0;
+    L->slice_stride = align_up(sizeof(double) * tc_wbuild_slice_doubles(v)) / sizeof(double);
     L->t2row_stride = align_up(sizeof(double) * O * V * LD) / sizeof(double);
     L->n_slots = o;
+    L->off_ovooT = take(sizeof(double) * O * O * V * (size_t)L->ldo);
+    if (mode != MODE_STREAMED && pad) L->off_t2 = take(sizeof(double) * O * L->t2row_stride);   // TMA needs 16-byte row strides
     if (mode == MODE_BLOCKS) {
-        if (pad) {   // TMA needs 16-byte row strides: zero-padded copies of the caller's arrays
-            L->off_t2 = take(sizeof(double) * O * L->t2row_stride);
-            L->off_ovoo = take(sizeof(double) * O * O * O * LD);
-            L->off_vvvo = take(sizeof(double) * O * L->slice_stride);
-        }
+        L->off_vvvo = take(sizeof(double) * O * L->slice_stride);
     } else {
-        if (mode == MODE_DF && pad) L->off_t2 = take(sizeof(double) * O * L->t2row_stride);
-        L->off_ovoo = take(sizeof(double) * O * O * O * LD);
         L->off_ovov = take(sizeof(double) * O * O * V * V);
         const size_t per_slot = sizeof(double) * (L->slice_stride + (mode == MODE_STREAMED ? L->t2row_stride : 0));
         long long slots = o;
@@ -109,6 +107,8 @@ tc_status check_common(tc_ctx* ctx, int o, int v, const double* eps_occ, const d
     if (!is_device_ptr(eps_occ) || !is_device_ptr(eps_vir) || !is_device_ptr(t1))
         TC_FAIL(ctx, TC_ERR_INVALID_ARG, "eps_occ, eps_vir, t1 must be device pointers");
     if (!t2_on_host && !is_device_ptr(t2)) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "t2 must be a device pointer");
+    if (!t2_on_host && (uintptr_t)t2 % 16 != 0)
+        TC_FAIL(ctx, TC_ERR_INVALID_ARG, "t2 must be 16-byte aligned (TMA operand; every CUDA allocator returns at least 256-byte alignment)");
     if (t2_on_host && (!t2 || is_device_ptr(t2))) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "t2_host must be a host pointer");
     if (blocks && (!is_device_ptr(blocks->vvvo) || !is_device_ptr(blocks->ovoo) || !is_device_ptr(blocks->ovov)))
         TC_FAIL(ctx, TC_ERR_INVALID_ARG, "blocks->vvvo/ovoo/ovov must be device pointers");
@@ -126,19 +126,25 @@ void fill_orbits(int v, std::vector<int4>& orb) {
             for (int C = 0; C <= B; C++) orb.push_back(make_int4(A, B, C, 0));
 }
 
-// ---- a2 launches: eq. (6) by the DMMA GEMM, outputs with row length ldv ----
-// slices x0 .. x0+nx-1 into dst (slice x at dst + (x - x0) * slice_stride, laid out [d][b][ldv])
-cudaError_t launch_slices(const tc_df_factors* df, int o, int v, int ldv, int x0, int nx, double* dst, size_t slice_stride,
-                          cudaStream_t st) {
-    // rows (d,b) -> d*v*ldv + b*ldv; cols (x,c) -> x*slice_stride + c
+// ---- a2 launches: eq. (6) by the DMMA GEMM ----
+// natural layouts (tc_build_blocks): slices x0 .. x0+nx-1 as [x][d][b][c]
+cudaError_t launch_slices_natural(const tc_df_factors* df, int o, int v, int x0, int nx, double* dst, cudaStream_t st) {
+    // rows (d,b) -> (d*v + b)*v; cols (x,c) -> x*v^3 + c
     return tc_launch_df_gemm(df->Bvv, (size_t)v * v, df->Bov + (size_t)x0 * v, (size_t)o * v, v * v, nx * v, df->naux,
-                             /*R2*/ v, /*sr1*/ (long long)v * ldv, /*sr2*/ ldv, /*C2*/ v, /*sc1*/ (long long)slice_stride, /*sc2*/ 1, dst, st);
+                             /*R2*/ 1, /*sr1*/ (long long)v, /*sr2*/ 0, /*C2*/ v, /*sc1*/ (long long)v * v * v, /*sc2*/ 1, dst, st);
 }
-cudaError_t launch_ovoo(const tc_df_factors* df, int o, int v, int ldv, double* dst, cudaStream_t st) {
-    // ovoo[j][k][l][c]: rows (l,j) -> l*ldv + j*o*o*ldv; cols (k,c) -> k*o*ldv + c
-    const long long O = o, LD = ldv;
-    return tc_launch_df_gemm(df->Boo, (size_t)(O * O), df->Bov, (size_t)(O * v), o * o, o * v, df->naux,
-                             /*R2*/ o, /*sr1*/ LD, /*sr2*/ O * O * LD, /*C2*/ v, /*sc1*/ O * LD, /*sc2*/ 1, dst, st);
+cudaError_t launch_ovoo_natural(const tc_df_factors* df, int o, int v, double* dst, cudaStream_t st) {
+    // ovoo[j][k][l][c]: rows (l,j) -> l*v + j*o*o*v; cols (k,c) -> k*o*v + c
+    const long long O = o, V = v;
+    return tc_launch_df_gemm(df->Boo, (size_t)(O * O), df->Bov, (size_t)(O * V), o * o, o * v, df->naux,
+                             /*R2*/ o, /*sr1*/ V, /*sr2*/ O * O * V, /*C2*/ v, /*sc1*/ O * V, /*sc2*/ 1, dst, st);
+}
+// the W-builder's hole A operand: (ov|oo)^T[z][x][m][ldo] = (l z | x m) = sum_Q Boo[Q][l][z] Bov[Q][x][m]
+cudaError_t launch_ovooT(const tc_df_factors* df, int o, int v, int ldo, double* dst, cudaStream_t st) {
+    // rows (l,z) -> l + z*o*v*ldo; cols (x,m) -> x*v*ldo + m*ldo
+    const long long O = o, V = v, LD = ldo;
+    return tc_launch_df_gemm(df->Boo, (size_t)(O * O), df->Bov, (size_t)(O * V), o * o, o * v, df->naux,
+                             /*R2*/ o, /*sr1*/ 1, /*sr2*/ O * V * LD, /*C2*/ v, /*sc1*/ V * LD, /*sc2*/ LD, dst, st);
 }
 cudaError_t launch_ovov(const tc_df_factors* df, int o, int v, double* dst, cudaStream_t st) {
     // ovov[j][k][b][c]: rows (j,b) -> j*o*v^2 + b*v; cols (k,c) -> k*v^2 + c
@@ -227,60 +233,48 @@ tc_status run_energy(tc_ctx* ctx, int o, int v, const double* eps_occ, const dou
     int n_tslots = o;
     const bool blocked = (mode == MODE_STREAMED) || (mode == MODE_DF && L.n_slots < o);
     TC_CUDA(ctx, cudaEventRecord(ctx->ev_s0, s));
+    double* w_ovooT = (double*)(ws + L.off_ovooT);
+    double* w_vvvo = (double*)(ws + L.off_vvvo);
+    a.ovooT = w_ovooT;
+    a.ldo = L.ldo;
+    a.slices = w_vvvo;
+    a.slice_stride = L.slice_stride;
+    a.ldv = ldv;
     if (mode == MODE_BLOCKS) {
+        // the caller's blocks, re-laid for the W-builder: slices tiled in fragment order, (ov|oo) with l fastest
         a.ovov = blocks->ovov;
-        if (pad) {
-            double* p_t2 = (double*)(ws + L.off_t2);
-            double* p_ovoo = (double*)(ws + L.off_ovoo);
-            double* p_vvvo = (double*)(ws + L.off_vvvo);
-            for (int x = 0; x < o; x++) {
-                TC_CUDA(ctx, tc_launch_pad_rows(p_t2 + (size_t)x * L.t2row_stride, ldv, t2 + (size_t)x * O * V * V, V, O * V, v, s));
-                TC_CUDA(ctx, tc_launch_pad_rows(p_vvvo + (size_t)x * L.slice_stride, ldv, blocks->vvvo + (size_t)x * V * V * V, V, V * V, v, s));
-            }
-            TC_CUDA(ctx, tc_launch_pad_rows(p_ovoo, ldv, blocks->ovoo, V, O * O * O, v, s));
-            ctx->stats.n_kernel_launches += 2 * o + 1;
-            a.t2 = p_t2;
-            a.ovoo = p_ovoo;
-            a.slices = p_vvvo;
-            a.slice_stride = L.slice_stride;
-            a.ldv = ldv;
-        } else {
-            a.t2 = t2;
-            a.ovoo = blocks->ovoo;
-            a.slices = blocks->vvvo;
-            a.slice_stride = V * V * V;
-            a.ldv = v;
-        }
+        for (int x = 0; x < o; x++) TC_CUDA(ctx, tc_launch_tile_slice(blocks->vvvo + (size_t)x * V * V * V, v, v, V, w_vvvo + (size_t)x * L.slice_stride, s));
+        TC_CUDA(ctx, tc_launch_transpose_ovoo(blocks->ovoo, o, v, L.ldo, w_ovooT, s));
+        ctx->stats.n_kernel_launches += o + 1;
     } else {
-        double* w_ovoo = (double*)(ws + L.off_ovoo);
         double* w_ovov = (double*)(ws + L.off_ovov);
-        double* w_vvvo = (double*)(ws + L.off_vvvo);
-        TC_CUDA(ctx, launch_ovoo(df, o, v, ldv, w_ovoo, s));
+        if (L.ldo != o) TC_CUDA(ctx, cudaMemsetAsync(w_ovooT, 0, sizeof(double) * O * O * V * (size_t)L.ldo, s));   // the pad column
+        TC_CUDA(ctx, launch_ovooT(df, o, v, L.ldo, w_ovooT, s));
         TC_CUDA(ctx, launch_ovov(df, o, v, w_ovov, s));
         ctx->stats.n_kernel_launches += 2;
+        // the GEMM writes the elements of a slice, not the zero padding of its tiles (ragged tiles, K rounded up to 4):
+        // clear the slots once per call
+        if (tc_wbuild_slice_doubles(v) != V * V * V)
+            TC_CUDA(ctx, cudaMemsetAsync(w_vvvo, 0, sizeof(double) * L.slice_stride * (size_t)L.n_slots, s));
         if (!blocked) {
             // all o slices in one launch
-            TC_CUDA(ctx, launch_slices(df, o, v, ldv, 0, o, w_vvvo, L.slice_stride, s));
+            TC_CUDA(ctx, tc_launch_df_slices_tiled(df->Bvv, df->Bov, o, v, df->naux, 0, o, w_vvvo, L.slice_stride, s));
             ctx->stats.n_kernel_launches++;
             ctx->stats.slices_built += o;
         }
-        a.ovoo = w_ovoo;
         a.ovov = w_ovov;
-        a.slices = w_vvvo;
-        a.slice_stride = L.slice_stride;
-        a.ldv = ldv;
-        if (mode == MODE_STREAMED) {
-            a.t2 = (double*)(ws + L.off_t2);   // amplitude-row slots [slot][y][a][ldv]
-            n_tslots = L.n_slots;
-        } else if (pad) {
-            double* p_t2 = (double*)(ws + L.off_t2);
-            for (int x = 0; x < o; x++)
-                TC_CUDA(ctx, tc_launch_pad_rows(p_t2 + (size_t)x * L.t2row_stride, ldv, t2 + (size_t)x * O * V * V, V, O * V, v, s));
-            ctx->stats.n_kernel_launches += o;
-            a.t2 = p_t2;
-        } else {
-            a.t2 = t2;
-        }
+    }
+    if (mode == MODE_STREAMED) {
+        a.t2 = (double*)(ws + L.off_t2);   // amplitude-row slots [slot][y][a][ldv]
+        n_tslots = L.n_slots;
+    } else if (pad) {
+        double* p_t2 = (double*)(ws + L.off_t2);
+        for (int x = 0; x < o; x++)
+            TC_CUDA(ctx, tc_launch_pad_rows(p_t2 + (size_t)x * L.t2row_stride, ldv, t2 + (size_t)x * O * V * V, V, O * V, v, s));
+        ctx->stats.n_kernel_launches += o;
+        a.t2 = p_t2;
+    } else {
+        a.t2 = t2;
     }
     TC_CUDA(ctx, cudaEventRecord(ctx->ev_s1, s));
     // amplitude rows: the caller's array has stride o*v*v, the padded copy / the slots sit at the aligned t2row_stride
@@ -294,9 +288,8 @@ tc_status run_energy(tc_ctx* ctx, int o, int v, const double* eps_occ, const dou
         TC_CUDA(ctx, cudaMemcpyAsync(d_orbits, orb.data(), sizeof(int4) * orb.size(), cudaMemcpyHostToDevice, s));
     }
     tc_wbuild_maps maps;
-    TC_CUDA(ctx, tc_wbuild_make_maps(a, blocked ? L.n_slots : o, n_tslots, &maps));
-    if (ctx->force_kernel == TC_KERNEL_CPASYNC) maps.valid = false;
-    int kernel_ran = 0;
+    TC_CUDA(ctx, tc_wbuild_make_maps(a, n_tslots, &maps));
+    if (!maps.valid) TC_FAIL(ctx, TC_ERR_INTERNAL, "tensor maps of the W-builder could not be encoded");
 
     TimingRing kring(ctx->ev_k0, ctx->ev_k1), gring(ctx->ev_g0, ctx->ev_g1);
     bool first_kernel = true, first_staging = true;
@@ -310,7 +303,7 @@ tc_status run_energy(tc_ctx* ctx, int o, int v, const double* eps_occ, const dou
         }
         a.recs = recs;
         a.n_trip = n;
-        TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits, s, &kernel_ran));
+        TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits, s));
         TC_CUDA(ctx, cudaEventRecord(ctx->ev_k1[slot], s));
         TC_CUDA(ctx, tc_launch_reduce_units(d_partial, n, L.n_orbits, dest, S_out, s));
         ctx->stats.n_kernel_launches += 2;
@@ -361,7 +354,6 @@ tc_status run_energy(tc_ctx* ctx, int o, int v, const double* eps_occ, const dou
         cudaStream_t side = ctx->side_stream;
         TC_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));         // the side stream starts after ovoo/ovov and the tables
         TC_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
-        double* w_vvvo = (double*)(ws + L.off_vvvo);
         double* w_t2 = (mode == MODE_STREAMED) ? (double*)(ws + L.off_t2) : nullptr;
         const long long nblocks = (long long)plan.blocks.size();
         for (long long n = 0; n < nblocks; n++) {
@@ -380,7 +372,7 @@ tc_status run_energy(tc_ctx* ctx, int o, int v, const double* eps_occ, const dou
                 }
                 for (int q = b.load_begin; q < b.load_end; q++) {
                     const tc_plan_load& ld = plan.loads[q];
-                    TC_CUDA(ctx, launch_slices(df, o, v, ldv, ld.x, 1, w_vvvo + (size_t)ld.slot * L.slice_stride, L.slice_stride, side));
+                    TC_CUDA(ctx, tc_launch_df_slices_tiled(df->Bvv, df->Bov, o, v, df->naux, ld.x, 1, w_vvvo + (size_t)ld.slot * L.slice_stride, L.slice_stride, side));
                     ctx->stats.n_kernel_launches++;
                     ctx->stats.slices_built++;
                     if (w_t2) {   // the amplitude row t2[x][:][:][:] from the host, padded on the fly when v is odd
@@ -441,7 +433,7 @@ tc_status run_energy(tc_ctx* ctx, int o, int v, const double* eps_occ, const dou
             ctx->stats.staging_last_ms = ms;
         }
     }
-    ctx->stats.kernel = kernel_ran;
+    ctx->stats.kernel = (count > 0) ? TC_KERNEL_TMA : 0;
     const long long nz = count - count_diagonal(o, first, count);
     ctx->stats.n_triplets = nz;
     ctx->stats.flop_contraction = (double)nz * 12.0 * (double)v * v * v * ((double)v + o);
@@ -481,12 +473,12 @@ extern "C" tc_status tc_build_blocks(tc_ctx* ctx, int o, int v, const tc_df_fact
     TC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
     if (vvvo_out && nx > 0) {
-        TC_CUDA(ctx, launch_slices(df, o, v, v, x0, nx, vvvo_out, (size_t)v * v * v, st));
+        TC_CUDA(ctx, launch_slices_natural(df, o, v, x0, nx, vvvo_out, st));
         ctx->stats.n_kernel_launches++;
         ctx->stats.slices_built += nx;
     }
     if (ovoo_out) {
-        TC_CUDA(ctx, launch_ovoo(df, o, v, v, ovoo_out, st));
+        TC_CUDA(ctx, launch_ovoo_natural(df, o, v, ovoo_out, st));
         ctx->stats.n_kernel_launches++;
     }
     if (ovov_out) {
@@ -576,14 +568,6 @@ extern "C" tc_status tc_triples_energy_host(tc_ctx* ctx, int o, int v, int naux,
     return st;
 }
 
-extern "C" tc_status tc_debug_force_kernel(tc_ctx* ctx, int which) {
-    if (!ctx) return TC_ERR_INVALID_ARG;
-    if (which != TC_KERNEL_AUTO && which != TC_KERNEL_TMA && which != TC_KERNEL_CPASYNC)
-        TC_FAIL(ctx, TC_ERR_INVALID_ARG, "unknown kernel selector %d", which);
-    ctx->force_kernel = which;
-    return TC_OK;
-}
-
 extern "C" tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j, int k, const double* t2,
                                         const tc_int_blocks* blocks, double* W_dev, void* stream) {
     if (!ctx) return TC_ERR_INVALID_ARG;
@@ -594,6 +578,7 @@ extern "C" tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j,
         TC_FAIL(ctx, TC_ERR_INVALID_ARG, "t2, blocks and W_dev must be device pointers");
     TC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t s = (cudaStream_t)stream;
+    if ((uintptr_t)t2 % 16 != 0) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "t2 must be 16-byte aligned");
     Layout L;
     make_layout(o, v, 0, MODE_BLOCKS, false, 0, &L);
     // debug path: scratch allocated here (not a compute call of the hot path); zeros stand in for eps and t1
@@ -601,7 +586,6 @@ extern "C" tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j,
     char* tmp = nullptr;
     TC_CUDA(ctx, cudaMalloc(&tmp, L.total + b_zero));
     const int ldv = L.ldv;
-    const bool pad = ldv != v;
     const size_t O = o, V = v;
     std::vector<int4> orb;
     fill_orbits(v, orb);
@@ -626,38 +610,33 @@ extern "C" tc_status tc_debug_W_triplet(tc_ctx* ctx, int o, int v, int i, int j,
     a.partial = (double*)(tmp + L.off_partial);
     a.n_orbits = L.n_orbits;
     a.W_debug = W_dev;
-    a.t2_row_stride = O * V * V;
-    if (pad) {
+    double* w_vvvo = (double*)(tmp + L.off_vvvo);
+    double* w_ovooT = (double*)(tmp + L.off_ovooT);
+    a.slices = w_vvvo;
+    a.slice_stride = L.slice_stride;
+    a.ovooT = w_ovooT;
+    a.ldo = L.ldo;
+    a.ldv = ldv;
+    for (int x = 0; x < o && e == cudaSuccess; x++)
+        if (x == i || x == j || x == k) e = tc_launch_tile_slice(blocks->vvvo + (size_t)x * V * V * V, v, v, V, w_vvvo + (size_t)x * L.slice_stride, s);
+    if (e == cudaSuccess) e = tc_launch_transpose_ovoo(blocks->ovoo, o, v, L.ldo, w_ovooT, s);
+    if (ldv != v) {
         double* p_t2 = (double*)(tmp + L.off_t2);
-        double* p_ovoo = (double*)(tmp + L.off_ovoo);
-        double* p_vvvo = (double*)(tmp + L.off_vvvo);
-        for (int x = 0; x < o && e == cudaSuccess; x++) {
+        for (int x = 0; x < o && e == cudaSuccess; x++)
             e = tc_launch_pad_rows(p_t2 + (size_t)x * L.t2row_stride, ldv, t2 + (size_t)x * O * V * V, V, O * V, v, s);
-            if (e == cudaSuccess && (x == i || x == j || x == k))
-                e = tc_launch_pad_rows(p_vvvo + (size_t)x * L.slice_stride, ldv, blocks->vvvo + (size_t)x * V * V * V, V, V * V, v, s);
-        }
-        if (e == cudaSuccess) e = tc_launch_pad_rows(p_ovoo, ldv, blocks->ovoo, V, O * O * O, v, s);
         a.t2 = p_t2;
-        a.ovoo = p_ovoo;
-        a.slices = p_vvvo;
-        a.slice_stride = L.slice_stride;
-        a.ldv = ldv;
         a.t2_row_stride = L.t2row_stride;
     } else {
         a.t2 = t2;
-        a.ovoo = blocks->ovoo;
-        a.slices = blocks->vvvo;
-        a.slice_stride = V * V * V;
-        a.ldv = v;
+        a.t2_row_stride = O * V * V;
     }
     if (e == cudaSuccess) {
         tc_wbuild_maps maps;
-        e = tc_wbuild_make_maps(a, o, o, &maps);
-        if (ctx->force_kernel == TC_KERNEL_CPASYNC) maps.valid = false;
-        int ran = 0;
-        if (e == cudaSuccess) e = tc_launch_wbuild(a, &maps, (const int4*)(tmp + L.off_orbits), s, &ran);
+        e = tc_wbuild_make_maps(a, o, &maps);
+        if (e == cudaSuccess && !maps.valid) e = cudaErrorInvalidValue;
+        if (e == cudaSuccess) e = tc_launch_wbuild(a, &maps, (const int4*)(tmp + L.off_orbits), s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-        ctx->stats.kernel = ran;
+        ctx->stats.kernel = TC_KERNEL_TMA;
     }
     cudaFree(tmp);
     if (e != cudaSuccess) TC_FAIL(ctx, TC_ERR_CUDA, "debug W kernel failed: %s", cudaGetErrorString(e));

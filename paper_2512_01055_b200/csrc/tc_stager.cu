@@ -8,6 +8,8 @@
 //     ovov[j][k][b][c] = sum_Q Bov[Q][j][b] Bov[Q][k][c]      M = o*v, N = o*v    (Fig. 2 l.16-18)
 // CTA tile 128 x 128, K chunk 16, 3-stage cp.async pipeline, 8 warps (4 x 2), warp tile 32 x 64
 // = 4 x 8 DMMA.8x8x4 blocks per k-step (12 fragment loads per 32 MMAs).
+#include <algorithm>
+
 #include "tc_common.cuh"
 
 namespace {
@@ -38,7 +40,12 @@ __device__ __forceinline__ void gemm_load(double (*dst)[LDS_], const double* src
     }
 }
 
-template <int VEC>
+// TILED = false: two-level linear output map.  TILED = true: rows are (d, b) = (row / v, row % v), columns (x, c) =
+// (col / v, col % v) of slice x, written in the W-builder's tiled layout
+//   [n1 tile b/16][n2 tile c/16][K chunk d/4][z = (c%16)/8][n1 = b%16][k = d%4][n2 = c%8]
+// (R2 = C2 = v, sr1 = tiles per edge nb, sr2 = K chunks nkq, sc1 = slice stride): a K chunk of a tile pair is then
+// 8 KB contiguous, in the fragment order of mma.sync m8n8k4, and the W-builder streams it with plain bulk copies.
+template <int VEC, bool TILED>
 __global__ void __launch_bounds__(GTHREADS, 1)
 k_df_gemm(const double* __restrict__ A, size_t lda, const double* __restrict__ B, size_t ldb, int M, int N, int K,
           int R2, long long sr1, long long sr2, int C2, long long sc1, long long sc2, double* __restrict__ C) {
@@ -94,14 +101,53 @@ k_df_gemm(const double* __restrict__ A, size_t lda, const double* __restrict__ B
     for (int x = 0; x < 4; x++) {
         const int row = m0 + wm * 32 + x * 8 + fr;
         if (row >= M) continue;
-        const long long roff = (long long)(row / R2) * sr1 + (long long)(row % R2) * sr2;
+        long long roff;
+        if (TILED) {
+            const int d = row / R2, b = row - d * R2;
+            roff = (((long long)(b >> 4) * sr1) * sr2 + (d >> 2)) * 1024 + (b & 15) * 32 + (d & 3) * 8;
+        } else {
+            roff = (long long)(row / R2) * sr1 + (long long)(row % R2) * sr2;
+        }
 #pragma unroll
         for (int y = 0; y < 8; y++)
 #pragma unroll
             for (int e = 0; e < 2; e++) {
                 const int col = n0 + wn * 64 + y * 8 + 2 * fk + e;
-                if (col < N) C[roff + (long long)(col / C2) * sc1 + (long long)(col % C2) * sc2] = acc[x][y][e];
+                if (col >= N) continue;
+                if (TILED) {
+                    const int xs = col / C2, c = col - xs * C2;
+                    C[roff + (long long)xs * sc1 + ((long long)(c >> 4) * sr2) * 1024 + ((c >> 3) & 1) * 512 + (c & 7)] = acc[x][y][e];
+                } else {
+                    C[roff + (long long)(col / C2) * sc1 + (long long)(col % C2) * sc2] = acc[x][y][e];
+                }
             }
+    }
+}
+
+// materialised src[k][b][c] (K rows, row length ld) -> tiled layout, padding included (one thread per destination element)
+__global__ void __launch_bounds__(256) k_tile_slice(const double* __restrict__ src, int K, int v, size_t ld, int nb, int nkq,
+                                                    double* __restrict__ dst) {
+    const size_t total = (size_t)nb * nb * nkq * 1024;
+    for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < total; n += (size_t)gridDim.x * blockDim.x) {
+        const int n2 = (int)(n & 7), k = (int)((n >> 3) & 3), n1 = (int)((n >> 5) & 15), z = (int)((n >> 9) & 1);
+        size_t t = n >> 10;
+        const int kq = (int)(t % nkq);
+        t /= nkq;
+        const int V = (int)(t % nb), U = (int)(t / nb);
+        const int d = kq * 4 + k, b = U * 16 + n1, c = V * 16 + z * 8 + n2;
+        dst[n] = (d < K && b < v && c < v) ? src[((size_t)d * v + b) * ld + c] : 0.0;
+    }
+}
+
+// ovoo[z][x][l][m] -> dst[z][x][m][ldo] (l fastest, pad zeroed)
+__global__ void __launch_bounds__(256) k_transpose_ovoo(const double* __restrict__ src, int o, int v, int ldo, size_t npanels,
+                                                        double* __restrict__ dst) {
+    const size_t per = (size_t)v * ldo, total = npanels * per;
+    for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < total; n += (size_t)gridDim.x * blockDim.x) {
+        const size_t panel = n / per;
+        const int r = (int)(n - panel * per);
+        const int m = r / ldo, l = r - m * ldo;
+        dst[n] = (l < o) ? src[(panel * o + l) * v + m] : 0.0;
     }
 }
 
@@ -109,9 +155,11 @@ k_df_gemm(const double* __restrict__ A, size_t lda, const double* __restrict__ B
 
 // per device: called by tc_create with the device current
 cudaError_t tc_stager_configure() {
-    cudaError_t e = cudaFuncSetAttribute(k_df_gemm<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_df_gemm<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    cudaError_t e = cudaFuncSetAttribute(k_df_gemm<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    return e;
 }
 
 cudaError_t tc_launch_df_gemm(const double* A, size_t lda, const double* B, size_t ldb, int M, int N, int K,
@@ -122,8 +170,40 @@ cudaError_t tc_launch_df_gemm(const double* A, size_t lda, const double* B, size
     if (grid.y > 65535) return cudaErrorInvalidConfiguration;
     const bool vec2 = (lda % 2 == 0) && (ldb % 2 == 0) && (((uintptr_t)A | (uintptr_t)B) % 16 == 0);
     if (vec2)
-        k_df_gemm<2><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(A, lda, B, ldb, M, N, K, R2, sr1, sr2, C2, sc1, sc2, C);
+        k_df_gemm<2, false><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(A, lda, B, ldb, M, N, K, R2, sr1, sr2, C2, sc1, sc2, C);
     else
-        k_df_gemm<1><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(A, lda, B, ldb, M, N, K, R2, sr1, sr2, C2, sc1, sc2, C);
+        k_df_gemm<1, false><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(A, lda, B, ldb, M, N, K, R2, sr1, sr2, C2, sc1, sc2, C);
+    return cudaGetLastError();
+}
+
+cudaError_t tc_launch_df_slices_tiled(const double* Bvv, const double* Bov, int o, int v, int naux, int x0, int nx, double* dst,
+                                      size_t slice_stride, cudaStream_t stream) {
+    if (nx <= 0) return cudaSuccess;
+    const int M = v * v, N = nx * v;
+    const size_t lda = (size_t)v * v, ldb = (size_t)o * v;
+    const double* B = Bov + (size_t)x0 * v;
+    dim3 grid((N + BN - 1) / BN, (M + BM - 1) / BM);
+    if (grid.y > 65535) return cudaErrorInvalidConfiguration;
+    const int nb = (v + 15) / 16, nkq = (v + 3) / 4;
+    const bool vec2 = (lda % 2 == 0) && (ldb % 2 == 0) && (((uintptr_t)Bvv | (uintptr_t)B) % 16 == 0);
+    if (vec2)
+        k_df_gemm<2, true><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(Bvv, lda, B, ldb, M, N, naux, v, nb, nkq, v, (long long)slice_stride, 0, dst);
+    else
+        k_df_gemm<1, true><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(Bvv, lda, B, ldb, M, N, naux, v, nb, nkq, v, (long long)slice_stride, 0, dst);
+    return cudaGetLastError();
+}
+
+cudaError_t tc_launch_tile_slice(const double* src, int K, int v, size_t ld, double* dst, cudaStream_t stream) {
+    const int nb = (v + 15) / 16, nkq = (K + 3) / 4;
+    const size_t total = (size_t)nb * nb * nkq * 1024;
+    const unsigned grid = (unsigned)std::min<size_t>((total + 255) / 256, 148 * 32);
+    k_tile_slice<<<grid, 256, 0, stream>>>(src, K, v, ld, nb, nkq, dst);
+    return cudaGetLastError();
+}
+
+cudaError_t tc_launch_transpose_ovoo(const double* ovoo, int o, int v, int ldo, double* dst, cudaStream_t stream) {
+    const size_t npanels = (size_t)o * o, total = npanels * v * ldo;
+    const unsigned grid = (unsigned)std::min<size_t>((total + 255) / 256, 148 * 32);
+    k_transpose_ovoo<<<grid, 256, 0, stream>>>(ovoo, o, v, ldo, npanels, dst);
     return cudaGetLastError();
 }

@@ -39,3 +39,11 @@ def read_golden_S(name):
             elif t[0] == "E":
                 E = float(t[1])
     return rows, E
+
+
+def tiled_slice_bytes(v):
+    """Bytes of one (vv|v.) slice slot in the library's workspace: the slice in the W-builder's tiled layout
+    ([n1 tile][n2 tile][K chunk][2][16][4][8] doubles, zero padded), rounded up to 256 (csrc/tc_energy.cu make_layout)."""
+    nb, nkq = (v + 15) // 16, (v + 3) // 4
+    return (nb * nb * nkq * 1024 * 8 + 255) // 256 * 256
+
