@@ -38,7 +38,13 @@ extern "C" tc_status tc_create(tc_ctx** out, int device) {
     ctx->l2_bytes = (size_t)prop.l2CacheSize;
     ctx->err[0] = 0;
     bool ok = cudaSetDevice(device) == cudaSuccess;
-    ok = ok && cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking) == cudaSuccess;
+    {
+        // the staging stream outranks the caller's: its GEMM CTAs are dispatched as soon as SMs free up, so the operands of
+        // block n+1 are in place long before the W-builder of block n (hundreds of thousands of queued CTAs) has drained
+        int prio_least = 0, prio_greatest = 0;
+        ok = ok && cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest) == cudaSuccess;
+        ok = ok && cudaStreamCreateWithPriority(&ctx->side_stream, cudaStreamNonBlocking, prio_greatest) == cudaSuccess;
+    }
     ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
     for (int n = 0; n < TC_EV_RING; n++) {
         ok = ok && cudaEventCreateWithFlags(&ctx->ev_staged[n], cudaEventDisableTiming) == cudaSuccess;

@@ -299,6 +299,32 @@ def test_deterministic_odd_v(ctx):
     assert E1 == E2 and (S1 == S2).all()
 
 
+def test_workspace_canaries(ctx):
+    """Bounds check of our own (compute-sanitizer is closed on this pool): guard bands before and after the workspace,
+    around S_dev and copies of the read-only inputs must be untouched by the calls, resident and blocked regime."""
+    p = harness.make_problem(9, 50, 10, 23, sigma_B=0.25, blocks=True)
+    dp = DevProblem(p)
+    o, v, naux = p.o, p.v, p.naux
+    n = oracle.triplet_count(o)
+    E_ref, S_ref = oracle.triples_energy(p)
+    guard = 1 << 16
+    full = ctx.workspace_bytes(o, v, naux)
+    small = ctx.workspace_bytes(o, v, naux, full - (o - 4) * harness.tiled_slice_bytes(v))
+    t2_copy, Bvv_copy = dp.t2.clone(), dp.Bvv.clone()
+    for nb in (full, small):
+        buf = torch.full((nb + 2 * guard,), 0xA5, dtype=torch.uint8, device="cuda")
+        Sbuf = torch.full((n + 64,), 12345.0, dtype=torch.float64, device="cuda")
+        ws = buf[guard:guard + nb]
+        assert ws.data_ptr() % 256 == 0
+        E = ctx.triples_energy_slice(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws, workspace_bytes=nb,
+                                     first=0, count=n, S_dev=Sbuf[32:32 + n])
+        assert_energy(E, E_ref)
+        assert bool((buf[:guard] == 0xA5).all()) and bool((buf[guard + nb:] == 0xA5).all())
+        assert bool((Sbuf[:32] == 12345.0).all()) and bool((Sbuf[32 + n:] == 12345.0).all())
+        assert np.abs(Sbuf[32:32 + n].cpu().numpy() - S_ref).max() <= REL_TOL * np.abs(S_ref).max()
+    assert torch.equal(t2_copy, dp.t2) and torch.equal(Bvv_copy, dp.Bvv)
+
+
 def test_argument_errors(ctx):
     from paper_2512_01055_b200.binding import TcError
     p = harness.make_problem(3, 8, 4, 3, blocks=True)
