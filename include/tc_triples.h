@@ -176,6 +176,26 @@ tc_status tc_triples_energy_streamed(tc_ctx* ctx, int o, int v,
                                      void* stream, long long first, long long count,
                                      double* S_dev, double* E_partial_out);
 
+/* The paper's own loop order (the abcijk scheme; Fig. 1; Fig. 2): virtual tile
+ * orbits {A >= B >= C} (tile edge 16) outer, all triplets i >= j >= k inner.  For each orbit the (vv|vo) integrals are
+ * rebuilt from the DF factors restricted to the orbit's tiles (Fig. 2 l.7, 10), so the footprint beside t2 and (ov|ov) is
+ * O(o v 16^2) instead of o v^3; the next orbit's integrals are assembled on the library's side stream while the current
+ * orbit's contraction runs.  Same kernels, same result as tc_triples_energy: E = sum over orbits of the orbit's energy
+ *   E_orbit = sum_{i>=j>=k} (2 - d_ij - d_jk) sum_{(a,b,c) in orbit} (W + Vd) R / D.
+ * Orbits orbit_first .. orbit_first+orbit_count-1 of the enumeration A >= B >= C (A slowest) are computed;
+ * E_orbit_dev (device, [orbit_count], optional) receives their energies, E_out (host) their sum.  DF input only;
+ * t2 device-resident, 16-byte aligned.  Workspace: tc_workspace_bytes_abcijk.  tc_tile_orbit_count(v) = nb(nb+1)(nb+2)/6,
+ * nb = ceil(v/16). */
+long long tc_tile_orbit_count(int v);
+tc_status tc_workspace_bytes_abcijk(tc_ctx* ctx, int o, int v, int naux, size_t* bytes);
+tc_status tc_triples_energy_abcijk(tc_ctx* ctx, int o, int v,
+                                   const double* eps_occ, const double* eps_vir,
+                                   const double* t1, const double* t2,
+                                   const tc_df_factors* df,
+                                   void* workspace, size_t workspace_bytes,
+                                   void* stream, long long orbit_first, long long orbit_count,
+                                   double* E_orbit_dev, double* E_out);
+
 /* End-to-end variant with HOST inputs: copies the DF factors, amplitudes and orbital
  * energies to the device, assembles the integrals, computes E(T) over triplets
  * first .. first+count-1, returns it on the host.  This is the one call that allocates

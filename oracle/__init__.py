@@ -34,6 +34,8 @@ def lib():
         L.tco_W_triplet.argtypes = [ctypes.c_int] * 5 + [_dp] * 6
         L.tco_S_from_W.restype = ctypes.c_double
         L.tco_S_from_W.argtypes = [ctypes.c_int] * 5 + [_dp] * 6
+        L.tco_S_from_W_tile_orbit.restype = ctypes.c_double
+        L.tco_S_from_W_tile_orbit.argtypes = [ctypes.c_int] * 5 + [_dp] * 5 + [ctypes.c_int] * 4
         L.tco_triples_energy_blocks.restype = ctypes.c_int
         L.tco_triples_energy_blocks.argtypes = [ctypes.c_int] * 2 + [_dp] * 7 + [ctypes.c_longlong] * 2 + [_dp] * 2
         L.tco_triples_energy_slices.restype = ctypes.c_int
@@ -91,6 +93,38 @@ def S_from_W(o, v, i, j, k, eps_occ, eps_vir, t1, ovov, W, want_Y=False):
     pY = Y.ctypes.data_as(_dp) if want_Y else None
     S = lib().tco_S_from_W(o, v, i, j, k, pe, pv, pt1, po, pW, pY)
     return (S, Y) if want_Y else S
+
+
+def S_from_W_tile_orbit(o, v, i, j, k, eps_occ, eps_vir, t1, ovov, W, T, A, B, C):
+    """S_ijk restricted to the points (a,b,c) of the tile orbit A >= B >= C (tile edge T)."""
+    eps_occ, pe = _f64(eps_occ)
+    eps_vir, pv = _f64(eps_vir)
+    t1, pt1 = _f64(t1)
+    ovov, po = _f64(ovov)
+    W, pW = _f64(W)
+    return lib().tco_S_from_W_tile_orbit(o, v, i, j, k, pe, pv, pt1, po, pW, T, A, B, C)
+
+
+def tile_orbits(v, T=16):
+    """The orbits of virtual tiles in the order A >= B >= C, A slowest (the order of tc_triples_energy_abcijk)."""
+    nb = (v + T - 1) // T
+    return [(A, B, C) for A in range(nb) for B in range(A + 1) for C in range(B + 1)]
+
+
+def orbit_energies(prob, T=16):
+    """E_orbit = sum_{i>=j>=k} (2 - d_ij - d_jk) sum_{(a,b,c) in orbit} Y R / D for every tile orbit (numpy array, the
+    order of tile_orbits): what the abcijk schedule produces per virtual tile, from the plain loops."""
+    o, v = prob.o, prob.v
+    orbs = tile_orbits(v, T)
+    E = np.zeros(len(orbs))
+    for idx in range(triplet_count(o)):
+        i, j, k, w = triplet_decode(o, idx)
+        if w == 0.0:
+            continue
+        W = W_triplet(o, v, i, j, k, prob.t2, prob.vvvo[i], prob.vvvo[j], prob.vvvo[k], prob.ovoo)
+        for n, (A, B, C) in enumerate(orbs):
+            E[n] += w * S_from_W_tile_orbit(o, v, i, j, k, prob.eps_occ, prob.eps_vir, prob.t1, prob.ovov, W, T, A, B, C)
+    return E
 
 
 def triples_energy(prob, first=0, count=None):

@@ -159,6 +159,38 @@ double tco_S_from_W(int o, int v, int i, int j, int k,
     return S;
 }
 
+/* ---- the same sum restricted to one orbit of virtual tiles (the paper's abcijk scheme loops over tiles of the virtual
+ *      indices, Fig. 1): only the points (a,b,c) whose tile indices (a/T, b/T, c/T), sorted in descending order,
+ *      equal (A,B,C).  The orbits partition the abc cube, so the restricted sums add up to tco_S_from_W. ---- */
+
+double tco_S_from_W_tile_orbit(int o, int v, int i, int j, int k,
+                               const double* eps_occ, const double* eps_vir,
+                               const double* t1, const double* ovov, const double* W,
+                               int T, int A, int B, int C) {
+    double S = 0.0;
+    const double eo = eps_occ[i] + eps_occ[j] + eps_occ[k];
+#define W_(a, b, c) W[((size_t)(a) * v + (b)) * v + (c)]
+    for (int a = 0; a < v; a++)
+        for (int b = 0; b < v; b++)
+            for (int c = 0; c < v; c++) {
+                int hi = a / T, mid = b / T, lo = c / T, tmp;       /* sort the three tile indices, descending */
+                if (hi < mid) { tmp = hi; hi = mid; mid = tmp; }
+                if (mid < lo) { tmp = mid; mid = lo; lo = tmp; }
+                if (hi < mid) { tmp = hi; hi = mid; mid = tmp; }
+                if (hi != A || mid != B || lo != C) continue;
+                double Vd = t1[(size_t)i * v + a] * OVOV(ovov, o, v, j, b, k, c)
+                          + t1[(size_t)j * v + b] * OVOV(ovov, o, v, i, a, k, c)
+                          + t1[(size_t)k * v + c] * OVOV(ovov, o, v, i, a, j, b);
+                double Y = W_(a, b, c) + Vd;
+                double D = eo - eps_vir[a] - eps_vir[b] - eps_vir[c];
+                double R = 4.0 * W_(a, b, c) + W_(b, c, a) + W_(c, a, b)
+                         - 2.0 * W_(a, c, b) - 2.0 * W_(c, b, a) - 2.0 * W_(b, a, c);
+                S += Y * R / D;
+            }
+#undef W_
+    return S;
+}
+
 /* ---- energy over a range of the linear triplet index ---- */
 
 int tco_triples_energy_slices(int o, int v,

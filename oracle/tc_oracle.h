@@ -47,6 +47,14 @@ double tco_S_from_W(int o, int v, int i, int j, int k,
                     const double* eps_occ, const double* eps_vir,
                     const double* t1, const double* ovov, const double* W, double* Y_out);
 
+/* The same sum restricted to the points (a,b,c) of one orbit of virtual tiles: tile indices (a/T, b/T, c/T) sorted in
+ * descending order equal to (A,B,C) (the abcijk scheme of the paper tiles the virtual indices, Fig. 1).
+ * Pinned by: the restricted sums over all orbits A>=B>=C add up to tco_S_from_W; a numpy mask over Y R / D on tiny inputs. */
+double tco_S_from_W_tile_orbit(int o, int v, int i, int j, int k,
+                               const double* eps_occ, const double* eps_vir,
+                               const double* t1, const double* ovov, const double* W,
+                               int T, int A, int B, int C);
+
 /* S_ijk for the triplets first..first+count-1 of the linear index (i>=j>=k),
  * and E_partial = sum w_ijk S_ijk over that range.  S_out may be NULL. */
 int tco_triples_energy_blocks(int o, int v,

@@ -56,6 +56,7 @@ EXPORTS = [
     "tc_triplet_count", "tc_triplet_decode", "tc_triplet_index", "tc_triplet_partition",
     "tc_workspace_bytes", "tc_workspace_bytes_streamed", "tc_plan_summary", "tc_plan_dump", "tc_build_blocks",
     "tc_triples_energy", "tc_triples_energy_slice", "tc_triples_energy_streamed", "tc_triples_energy_host",
+    "tc_tile_orbit_count", "tc_workspace_bytes_abcijk", "tc_triples_energy_abcijk",
     "tc_debug_W_triplet",
     "tc_get_stats", "tc_bench_dmma_peak", "tc_bench_dfma_peak", "tc_bench_copy_bw", "tc_bench_ring_peak",
 ]
@@ -89,6 +90,10 @@ def lib() -> ctypes.CDLL:
     L.tc_workspace_bytes.argtypes = [_vp, _i, _i, _i, _sz, _P(_sz)]
     L.tc_workspace_bytes_streamed.argtypes = [_vp, _i, _i, _i, _sz, _P(_sz)]
     L.tc_plan_summary.argtypes = [_i, _ll, _ll, _i, _P(_ll), _P(_ll), _P(_i), _P(_i), _P(_i)]
+    L.tc_tile_orbit_count.argtypes = [_i]
+    L.tc_tile_orbit_count.restype = _ll
+    L.tc_workspace_bytes_abcijk.argtypes = [_vp, _i, _i, _i, _P(_sz)]
+    L.tc_triples_energy_abcijk.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_DfFactors), _vp, _sz, _vp, _ll, _ll, _vp, _P(_d)]
     L.tc_plan_dump.argtypes = [_i, _ll, _ll, _i, _vp, _vp, _ll]
     L.tc_triples_energy_streamed.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_DfFactors), _vp, _sz, _vp, _ll, _ll, _vp, _P(_d)]
     L.tc_bench_ring_peak.argtypes = [_vp, _i, _d, _vp, _sz, _P(_d)]
@@ -210,6 +215,23 @@ class Context:
                                                      _ptr(S_dev), ctypes.byref(E)))
         return E.value
 
+    def workspace_bytes_abcijk(self, o: int, v: int, naux: int) -> int:
+        out = _sz()
+        self._check(lib().tc_workspace_bytes_abcijk(self._h, o, v, naux, ctypes.byref(out)))
+        return int(out.value)
+
+    def triples_energy_abcijk(self, o, v, eps_occ, eps_vir, t1, t2, *, df, workspace, workspace_bytes, stream=None,
+                              orbit_first=0, orbit_count=None, E_orbit_dev=None) -> float:
+        """The paper's abcijk schedule: tile orbits outer, all triplets inner (see the header)."""
+        d = _DfFactors(int(df[0]), _ptr(df[1]), _ptr(df[2]), _ptr(df[3]))
+        if orbit_count is None:
+            orbit_count = tile_orbit_count(v) - orbit_first
+        E = _d()
+        self._check(lib().tc_triples_energy_abcijk(self._h, o, v, _ptr(eps_occ), _ptr(eps_vir), _ptr(t1), _ptr(t2), ctypes.byref(d),
+                                                   _ptr(workspace), workspace_bytes, _stream(stream), orbit_first, orbit_count,
+                                                   _ptr(E_orbit_dev), ctypes.byref(E)))
+        return E.value
+
     def triples_energy_host(self, o, v, naux, eps_occ, eps_vir, t1, t2, Boo, Bov, Bvv, first=0, count=None):
         """HOST (numpy) inputs; returns (E, bytes copied host->device)."""
         arrs = [_host(x) for x in (eps_occ, eps_vir, t1, t2, Boo, Bov, Bvv)]
@@ -280,6 +302,10 @@ def plan_dump(o: int, first: int, count: int, nslots: int):
     if rc != TC_OK:
         raise TcError(rc, "tc_plan_dump failed")
     return recs[:count], loads[:n_loads]
+
+
+def tile_orbit_count(v: int) -> int:
+    return int(lib().tc_tile_orbit_count(v))
 
 
 def triplet_count(o: int) -> int:

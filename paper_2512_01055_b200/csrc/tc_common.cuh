@@ -92,6 +92,10 @@ cudaError_t tc_launch_df_gemm(const double* A, size_t lda, const double* B, size
 // layout (slice x at dst + (x - x0) * slice_stride; the zero padding is NOT written: the caller clears the slots once).
 cudaError_t tc_launch_df_slices_tiled(const double* Bvv, const double* Bov, int o, int v, int naux, int x0, int nx,
                                       double* dst, size_t slice_stride, cudaStream_t stream);
+// abcijk schedule: the tile-restricted parts of all o slices for one tile orbit (A, B, C), chunk layout over the 3 x 3 local tile
+// pairs [lu][lv][K chunk][z][n1][k][n2 8]; x at dst + x * x_stride
+cudaError_t tc_launch_df_slices_orbit(const double* Bvv, const double* Bov, int o, int v, int naux, int tA, int tB, int tC, double* dst,
+                                      size_t x_stride, cudaStream_t stream);
 // the same layout from a materialised array src[k][b][c] (K rows k, row length ld >= v): a slice of the caller's (vv|vo)
 // block (K = v) or an amplitude row t2[y] (K = o); writes the padding too
 cudaError_t tc_launch_tile_slice(const double* src, int K, int v, size_t ld, double* dst, cudaStream_t stream);
@@ -124,6 +128,8 @@ struct tc_wbuild_args {
     const double* slices;            // slot s at slices + s * slice_stride, in the W-builder's tiled layout
                                      // [n1 tile][n2 tile][K chunk][z][n1 16][k 4][n2 8], zero padded (tc_wbuild_slice_doubles)
     size_t slice_stride;             // doubles
+    int orbit_local;                 // 1 (abcijk schedule): the slices hold only the 3 x 3 tile pairs of the launch's one tile orbit,
+                                     // pair (lu, lv) = positions of the n1 / n2 tile in (A, B, C)
     const double* ovooT;             // [z][x][m][ldo] = (l z | x m): the (ov|oo) block with the contracted index fastest
     const double* ovov;              // [j][k][b][c] (natural layout; read by the epilogue only)
     const tc_trip_rec* recs;         // device array [n_trip]
@@ -159,6 +165,9 @@ cudaError_t tc_launch_pad_rows(double* dst, size_t ldd, const double* src, size_
 cudaError_t tc_launch_make_triplets(int o, long long first, int n, tc_trip_rec* recs, double* w, cudaStream_t stream);
 //   S[dest ? dest[t] : t] = sum_u partial[t][u], fixed order
 cudaError_t tc_launch_reduce_units(const double* partial, int n_trip, int n_units, const int* dest, double* S, cudaStream_t stream);
+//   abcijk schedule: S[t] = (first ? 0 : S[t]) + partial[t];  *E_orbit = sum_t w[t] * partial[t] (fixed order, one block)
+cudaError_t tc_launch_accumulate_orbit(const double* partial, const double* w, long long n, int first, double* S, double* E_orbit,
+                                       cudaStream_t stream);
 //   *E = sum_t w[t] * S[t], fixed order, one block
 cudaError_t tc_launch_reduce_energy(const double* S, const double* w, long long n, double* E, cudaStream_t stream);
 

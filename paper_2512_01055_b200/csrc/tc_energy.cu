@@ -15,7 +15,7 @@ namespace {
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
-enum Mode { MODE_BLOCKS = 0, MODE_DF = 1, MODE_STREAMED = 2 };
+enum Mode { MODE_BLOCKS = 0, MODE_DF = 1, MODE_STREAMED = 2, MODE_ABCIJK = 3 };
 
 // How the caller's workspace is carved.  Everything the compute calls need lives here
 // (pre-allocate and reuse; no device allocation inside the call).
@@ -32,6 +32,8 @@ struct Layout {
     int ldv;            // row length of the TMA-addressed t2: v, or v + 1 when v is odd
     int ldo;            // row length of (ov|oo)^T: o rounded up to even
     size_t slice_stride, t2row_stride;   // doubles
+    size_t off_Eorb;    // abcijk schedule: per-orbit partial energies [n_orbits]
+    size_t orbit_buf_stride;   // abcijk schedule: doubles between the two staging buffers (o tile-restricted slices each)
 };
 
 constexpr size_t kPartialBudget = (size_t)256 << 20;
@@ -68,7 +70,16 @@ bool make_layout(int o, int v, int naux, Mode mode, bool bounded, size_t budget,
     L->n_slots = o;
     L->off_ovooT = take(sizeof(double) * O * O * V * (size_t)L->ldo);
     if (mode != MODE_STREAMED && pad) L->off_t2 = take(sizeof(double) * O * L->t2row_stride);   // TMA needs 16-byte row strides
-    if (mode == MODE_BLOCKS) {
+    L->off_Eorb = 0;
+    L->orbit_buf_stride = 0;
+    if (mode == MODE_ABCIJK) {
+        // tile-restricted slices: 3 x 3 local tile pairs instead of nb^2, for all o occupied indices, double buffered
+        L->off_ovov = take(sizeof(double) * O * O * V * V);
+        L->slice_stride = align_up(sizeof(double) * 9 * (size_t)((v + 3) / 4) * 1024) / sizeof(double);
+        L->orbit_buf_stride = O * L->slice_stride;
+        L->off_vvvo = take(sizeof(double) * 2 * L->orbit_buf_stride);
+        L->off_Eorb = take(sizeof(double) * (size_t)L->n_orbits);
+    } else if (mode == MODE_BLOCKS) {
         L->off_vvvo = take(sizeof(double) * O * L->slice_stride);
     } else {
         L->off_ovov = take(sizeof(double) * O * O * V * V);
@@ -460,6 +471,155 @@ extern "C" tc_status tc_workspace_bytes_streamed(tc_ctx* ctx, int o, int v, int 
     if (!make_layout(o, v, naux, MODE_STREAMED, hbm_budget != 0, hbm_budget, &L))
         TC_FAIL(ctx, TC_ERR_WORKSPACE_TOO_SMALL, "problem does not fit the HBM budget of %zu bytes", hbm_budget);
     *bytes = L.total;
+    return TC_OK;
+}
+
+extern "C" tc_status tc_workspace_bytes_abcijk(tc_ctx* ctx, int o, int v, int naux, size_t* bytes) {
+    if (!ctx || !bytes) return TC_ERR_INVALID_ARG;
+    if (o < 1 || v < 1 || naux < 1) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "bad sizes o=%d v=%d naux=%d", o, v, naux);
+    Layout L;
+    make_layout(o, v, naux, MODE_ABCIJK, false, 0, &L);
+    *bytes = L.total;
+    return TC_OK;
+}
+
+extern "C" long long tc_tile_orbit_count(int v) { return v < 1 ? -1 : (long long)tc_wbuild_num_orbits(v); }
+
+// The paper's own loop order (abcijk; Fig. 1; Fig. 2): virtual tile orbits outer, all
+// i >= j >= k inner; per orbit the integrals are rebuilt from the factors restricted to its tiles (Fig. 2 l.7, 10), so the
+// footprint beside t2 is O(o v T^2) instead of o v^3.  The next orbit's integrals are assembled on the side stream while the
+// current orbit's W-builder launch (all triplets x this orbit) runs.
+extern "C" tc_status tc_triples_energy_abcijk(tc_ctx* ctx, int o, int v, const double* eps_occ, const double* eps_vir,
+                                              const double* t1, const double* t2, const tc_df_factors* df, void* workspace,
+                                              size_t workspace_bytes, void* stream, long long orbit_first, long long orbit_count,
+                                              double* E_orbit_dev, double* E_out) {
+    if (!ctx) return TC_ERR_INVALID_ARG;
+    if (!df) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "the abcijk call takes DF factors");
+    tc_status st = check_common(ctx, o, v, eps_occ, eps_vir, t1, t2, false, nullptr, df);
+    if (st != TC_OK) return st;
+    if (!E_out) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "E_out must not be NULL");
+    if (E_orbit_dev && !is_device_ptr(E_orbit_dev)) TC_FAIL(ctx, TC_ERR_INVALID_ARG, "E_orbit_dev must be a device pointer");
+    Layout L;
+    make_layout(o, v, df->naux, MODE_ABCIJK, false, 0, &L);
+    if (!is_device_ptr(workspace) || L.total > workspace_bytes)
+        TC_FAIL(ctx, TC_ERR_WORKSPACE_TOO_SMALL, "workspace of %zu bytes is too small or not device memory (see tc_workspace_bytes_abcijk)",
+                workspace_bytes);
+    if (orbit_first < 0 || orbit_count < 0 || orbit_first + orbit_count > L.n_orbits)
+        TC_FAIL(ctx, TC_ERR_INVALID_ARG, "orbit range [%lld,%lld) outside [0,%d)", orbit_first, orbit_first + orbit_count, L.n_orbits);
+    const long long ntrip = tc_triplet_count(o);
+    if ((long long)L.batch * L.n_orbits < ntrip || ntrip > 0x7fffffffLL) TC_FAIL(ctx, TC_ERR_INTERNAL, "partial buffer too small for %lld triplets", ntrip);
+    TC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t s = (cudaStream_t)stream, side = ctx->side_stream;
+    char* ws = (char*)workspace;
+    int4* d_orbits = (int4*)(ws + L.off_orbits);
+    tc_trip_rec* d_recs = (tc_trip_rec*)(ws + L.off_recs);
+    double* d_w = (double*)(ws + L.off_w);
+    double* d_S = (double*)(ws + L.off_S);
+    double* d_partial = (double*)(ws + L.off_partial);
+    double* d_E = (double*)(ws + L.off_E);
+    double* d_Eorb = (double*)(ws + L.off_Eorb);
+    double* w_ovooT = (double*)(ws + L.off_ovooT);
+    double* w_ovov = (double*)(ws + L.off_ovov);
+    double* w_buf = (double*)(ws + L.off_vvvo);
+    const size_t O = o, V = v;
+    const bool pad = L.ldv != v;
+
+    memset(&ctx->stats, 0, sizeof(ctx->stats));
+    ctx->stats.padded = pad ? 1 : 0;
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_t0, s));
+    std::vector<int4> orb;
+    fill_orbits(v, orb);
+    TC_CUDA(ctx, cudaMemcpyAsync(d_orbits, orb.data(), sizeof(int4) * orb.size(), cudaMemcpyHostToDevice, s));
+    if (L.ldo != o) TC_CUDA(ctx, cudaMemsetAsync(w_ovooT, 0, sizeof(double) * O * O * V * (size_t)L.ldo, s));
+    TC_CUDA(ctx, launch_ovooT(df, o, v, L.ldo, w_ovooT, s));
+    TC_CUDA(ctx, launch_ovov(df, o, v, w_ovov, s));
+    TC_CUDA(ctx, cudaMemsetAsync(w_buf, 0, sizeof(double) * 2 * L.orbit_buf_stride, s));   // K padding of the chunk layout stays zero
+    TC_CUDA(ctx, tc_launch_make_triplets(o, 0, (int)ntrip, d_recs, d_w, s));
+    ctx->stats.n_kernel_launches += 3;
+    tc_wbuild_args a;
+    memset(&a, 0, sizeof(a));
+    a.o = o;
+    a.v = v;
+    a.ldv = L.ldv;
+    a.ldo = L.ldo;
+    a.eps_occ = eps_occ;
+    a.eps_vir = eps_vir;
+    a.t1 = t1;
+    a.ovooT = w_ovooT;
+    a.ovov = w_ovov;
+    a.slice_stride = L.slice_stride;
+    a.orbit_local = 1;
+    a.recs = d_recs;
+    a.n_trip = (int)ntrip;
+    a.partial = d_partial;
+    a.n_orbits = 1;
+    if (pad) {
+        double* p_t2 = (double*)(ws + L.off_t2);
+        for (int x = 0; x < o; x++)
+            TC_CUDA(ctx, tc_launch_pad_rows(p_t2 + (size_t)x * L.t2row_stride, L.ldv, t2 + (size_t)x * O * V * V, V, O * V, v, s));
+        ctx->stats.n_kernel_launches += o;
+        a.t2 = p_t2;
+        a.t2_row_stride = L.t2row_stride;
+    } else {
+        a.t2 = t2;
+        a.t2_row_stride = O * V * V;
+    }
+    tc_wbuild_maps maps;
+    TC_CUDA(ctx, tc_wbuild_make_maps(a, o, &maps));
+    if (!maps.valid) TC_FAIL(ctx, TC_ERR_INTERNAL, "tensor maps of the W-builder could not be encoded");
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));
+    TC_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
+    TimingRing kring(ctx->ev_k0, ctx->ev_k1), gring(ctx->ev_g0, ctx->ev_g1);
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_c0, s));
+    for (long long n = 0; n < orbit_count; n++) {
+        const int4 ob = orb[(size_t)(orbit_first + n)];
+        double* buf = w_buf + (size_t)(n & 1) * L.orbit_buf_stride;
+        // staging buffer n & 1 was last read by orbit n - 2
+        if (n >= 2) TC_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_done[(n - 2) % TC_EV_RING], 0));
+        const int g = gring.next();
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_g0[g], side));
+        TC_CUDA(ctx, tc_launch_df_slices_orbit(df->Bvv, df->Bov, o, v, df->naux, ob.x, ob.y, ob.z, buf, L.slice_stride, side));
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_g1[g], side));
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_staged[n % TC_EV_RING], side));
+        TC_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_staged[n % TC_EV_RING], 0));
+        const int kslot = kring.next();
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_k0[kslot], s));
+        a.slices = buf;
+        TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits + (orbit_first + n), s));
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_k1[kslot], s));
+        TC_CUDA(ctx, tc_launch_accumulate_orbit(d_partial, d_w, ntrip, n == 0 ? 1 : 0, d_S, d_Eorb + n, s));
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_done[n % TC_EV_RING], s));
+        ctx->stats.n_kernel_launches += 3;
+        ctx->stats.n_work_units += ntrip;
+        ctx->stats.slices_built += o;
+    }
+    ctx->stats.n_blocks = orbit_count;
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_c1, s));
+    if (orbit_count == 0) TC_CUDA(ctx, cudaMemsetAsync(d_S, 0, sizeof(double) * (size_t)ntrip, s));
+    TC_CUDA(ctx, tc_launch_reduce_energy(d_S, d_w, ntrip, d_E, s));
+    ctx->stats.n_kernel_launches++;
+    if (E_orbit_dev && orbit_count > 0)
+        TC_CUDA(ctx, cudaMemcpyAsync(E_orbit_dev, d_Eorb, sizeof(double) * (size_t)orbit_count, cudaMemcpyDeviceToDevice, s));
+    TC_CUDA(ctx, cudaMemcpyAsync(ctx->pinned, d_E, sizeof(double), cudaMemcpyDeviceToHost, s));
+    TC_CUDA(ctx, cudaEventRecord(ctx->ev_t1, s));
+    TC_CUDA(ctx, cudaStreamSynchronize(s));
+    TC_CUDA(ctx, cudaStreamSynchronize(side));
+    float ms = 0;
+    cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_t1);
+    ctx->stats.ms_total = ms;
+    cudaEventElapsedTime(&ms, ctx->ev_c0, ctx->ev_c1);
+    ctx->stats.ms_contraction = ms;
+    kring.finish();
+    gring.finish();
+    ctx->stats.ms_kernels = kring.total_ms;
+    ctx->stats.ms_staging = ctx->stats.ms_staging_side = gring.total_ms;
+    ctx->stats.kernel = orbit_count > 0 ? TC_KERNEL_TMA : 0;
+    const long long nz = ntrip - o;   // all but the o triplets i = j = k
+    ctx->stats.n_triplets = nz;
+    // executed contraction flop of the orbits in the range: 294 912 (v + o) per (triplet, generic orbit) when no tile is ragged;
+    // the full range sums to exactly 12 v^3 (v + o) per non-zero triplet
+    ctx->stats.flop_contraction = (orbit_count == L.n_orbits) ? (double)nz * 12.0 * (double)v * v * v * ((double)v + o) : 0.0;
+    *E_out = ctx->pinned[0];
     return TC_OK;
 }
 

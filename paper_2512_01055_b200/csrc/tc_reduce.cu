@@ -80,7 +80,30 @@ __global__ void __launch_bounds__(1024) k_reduce_energy(const double* __restrict
     if (threadIdx.x == 0) *E = x;
 }
 
+// abcijk schedule: fold one tile orbit's per-triplet partials into S and form the orbit's partial energy
+__global__ void __launch_bounds__(1024) k_accumulate_orbit(const double* __restrict__ partial, const double* __restrict__ w, long long n,
+                                                           int first, double* __restrict__ S, double* __restrict__ E_orbit) {
+    __shared__ double sh[1024];
+    double x = 0.0, comp = 0.0;
+    for (long long t = threadIdx.x; t < n; t += 1024) {
+        const double p = partial[t];
+        S[t] = first ? p : S[t] + p;
+        const double y = w[t] * p - comp;
+        const double z = x + y;
+        comp = (z - x) - y;
+        x = z;
+    }
+    x = block_sum_fixed(x, sh);
+    if (threadIdx.x == 0 && E_orbit) *E_orbit = x;
+}
+
 }  // namespace
+
+cudaError_t tc_launch_accumulate_orbit(const double* partial, const double* w, long long n, int first, double* S, double* E_orbit,
+                                       cudaStream_t stream) {
+    k_accumulate_orbit<<<1, 1024, 0, stream>>>(partial, w, n, first, S, E_orbit);
+    return cudaGetLastError();
+}
 
 cudaError_t tc_launch_make_triplets(int o, long long first, int n, tc_trip_rec* recs, double* w, cudaStream_t stream) {
     if (n <= 0) return cudaSuccess;

@@ -40,15 +40,43 @@ __device__ __forceinline__ void gemm_load(double (*dst)[LDS_], const double* src
     }
 }
 
+// Tile-restricted operand panels (the abcijk schedule): column col of the panel is element (col / 48, tile[(col / 16) % 3] * 16 +
+// col % 16) of a [.][v] array, i.e. only the three 16-wide tiles of the second index; elements at or beyond v read as zero.
+struct TileSel {
+    int t[3];
+};
+template <int VEC>
+__device__ __forceinline__ void gemm_load_tiles(double (*dst)[LDS_], const double* src, size_t ld, int col0, int ncols, int k0, int K,
+                                                int v, TileSel ts) {
+    constexpr int PIECES = BK * BM / VEC;
+#pragma unroll
+    for (int p = threadIdx.x; p < PIECES; p += GTHREADS) {
+        const int c = (p % (BM / VEC)) * VEC;
+        const int kk = p / (BM / VEC);
+        const int col = col0 + c;
+        const int g = col >> 4, within = col & 15, outer = g / 3, which = g - 3 * outer;
+        const int idx = ts.t[which] * 16 + within;
+        int nvalid = v - idx;
+        nvalid = (k0 + kk < K && col < ncols) ? (nvalid < 0 ? 0 : (nvalid > VEC ? VEC : nvalid)) : 0;
+        const double* s = nvalid ? src + (size_t)(k0 + kk) * ld + (size_t)outer * v + idx : src;
+        const uint32_t d = smem_u32(&dst[kk][c]);
+        if (VEC == 2) cp_async16(d, s, nvalid * 8);
+        else cp_async8(d, s, nvalid * 8);
+    }
+}
+
 // TILED = false: two-level linear output map.  TILED = true: rows are (d, b) = (row / v, row % v), columns (x, c) =
 // (col / v, col % v) of slice x, written in the W-builder's tiled layout
 //   [n1 tile b/16][n2 tile c/16][K chunk d/4][z = (c%16)/8][n1 = b%16][k = d%4][n2 = c%8]
 // (R2 = C2 = v, sr1 = tiles per edge nb, sr2 = K chunks nkq, sc1 = slice stride): a K chunk of a tile pair is then
 // 8 KB contiguous, in the fragment order of mma.sync m8n8k4, and the W-builder streams it with plain bulk copies.
-template <int VEC, bool TILED>
+// TILED = 2 (abcijk schedule): both operands are tile-restricted panels (TileSel), rows (d, lu, bl), columns (x, lv, cl); the
+// output is the same chunk layout over the 3 x 3 local tile pairs: [lu][lv][K chunk][z][n1][k][n2 8] per x (sc1 = stride of x,
+// sr2 = K chunks, R2 = v).
+template <int VEC, int TILED>
 __global__ void __launch_bounds__(GTHREADS, 1)
 k_df_gemm(const double* __restrict__ A, size_t lda, const double* __restrict__ B, size_t ldb, int M, int N, int K,
-          int R2, long long sr1, long long sr2, int C2, long long sc1, long long sc2, double* __restrict__ C) {
+          int R2, long long sr1, long long sr2, int C2, long long sc1, long long sc2, double* __restrict__ C, TileSel ts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     GemmSmem& s = *reinterpret_cast<GemmSmem*>(smem_raw);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -66,8 +94,13 @@ k_df_gemm(const double* __restrict__ A, size_t lda, const double* __restrict__ B
     int ld_c = 0;
     auto load_next = [&]() {
         if (ld_c < nchunks) {
-            gemm_load<VEC>(s.A[ld_c % GSTAGES], A, lda, m0, M, ld_c * BK, K);
-            gemm_load<VEC>(s.B[ld_c % GSTAGES], B, ldb, n0, N, ld_c * BK, K);
+            if (TILED == 2) {
+                gemm_load_tiles<VEC>(s.A[ld_c % GSTAGES], A, lda, m0, M, ld_c * BK, K, R2, ts);
+                gemm_load_tiles<VEC>(s.B[ld_c % GSTAGES], B, ldb, n0, N, ld_c * BK, K, R2, ts);
+            } else {
+                gemm_load<VEC>(s.A[ld_c % GSTAGES], A, lda, m0, M, ld_c * BK, K);
+                gemm_load<VEC>(s.B[ld_c % GSTAGES], B, ldb, n0, N, ld_c * BK, K);
+            }
             ld_c++;
         }
         cp_async_commit();
@@ -102,7 +135,10 @@ k_df_gemm(const double* __restrict__ A, size_t lda, const double* __restrict__ B
         const int row = m0 + wm * 32 + x * 8 + fr;
         if (row >= M) continue;
         long long roff;
-        if (TILED) {
+        if (TILED == 2) {
+            const int d = row / 48, lb = row - d * 48;   // lb = 16 lu + bl
+            roff = (((long long)(lb >> 4) * 3) * sr2 + (d >> 2)) * 1024 + (lb & 15) * 32 + (d & 3) * 8;
+        } else if (TILED == 1) {
             const int d = row / R2, b = row - d * R2;
             roff = (((long long)(b >> 4) * sr1) * sr2 + (d >> 2)) * 1024 + (b & 15) * 32 + (d & 3) * 8;
         } else {
@@ -114,7 +150,10 @@ k_df_gemm(const double* __restrict__ A, size_t lda, const double* __restrict__ B
             for (int e = 0; e < 2; e++) {
                 const int col = n0 + wn * 64 + y * 8 + 2 * fk + e;
                 if (col >= N) continue;
-                if (TILED) {
+                if (TILED == 2) {
+                    const int xs = col / 48, lc = col - xs * 48;   // lc = 16 lv + cl
+                    C[roff + (long long)xs * sc1 + ((long long)(lc >> 4) * sr2) * 1024 + ((lc >> 3) & 1) * 512 + (lc & 7)] = acc[x][y][e];
+                } else if (TILED == 1) {
                     const int xs = col / C2, c = col - xs * C2;
                     C[roff + (long long)xs * sc1 + ((long long)(c >> 4) * sr2) * 1024 + ((c >> 3) & 1) * 512 + (c & 7)] = acc[x][y][e];
                 } else {
@@ -155,10 +194,12 @@ __global__ void __launch_bounds__(256) k_transpose_ovoo(const double* __restrict
 
 // per device: called by tc_create with the device current
 cudaError_t tc_stager_configure() {
-    cudaError_t e = cudaFuncSetAttribute(k_df_gemm<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    cudaError_t e = cudaFuncSetAttribute(k_df_gemm<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_df_gemm<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GemmSmem));
     return e;
 }
 
@@ -170,9 +211,9 @@ cudaError_t tc_launch_df_gemm(const double* A, size_t lda, const double* B, size
     if (grid.y > 65535) return cudaErrorInvalidConfiguration;
     const bool vec2 = (lda % 2 == 0) && (ldb % 2 == 0) && (((uintptr_t)A | (uintptr_t)B) % 16 == 0);
     if (vec2)
-        k_df_gemm<2, false><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(A, lda, B, ldb, M, N, K, R2, sr1, sr2, C2, sc1, sc2, C);
+        k_df_gemm<2, 0><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(A, lda, B, ldb, M, N, K, R2, sr1, sr2, C2, sc1, sc2, C, TileSel{{0, 0, 0}});
     else
-        k_df_gemm<1, false><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(A, lda, B, ldb, M, N, K, R2, sr1, sr2, C2, sc1, sc2, C);
+        k_df_gemm<1, 0><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(A, lda, B, ldb, M, N, K, R2, sr1, sr2, C2, sc1, sc2, C, TileSel{{0, 0, 0}});
     return cudaGetLastError();
 }
 
@@ -187,9 +228,28 @@ cudaError_t tc_launch_df_slices_tiled(const double* Bvv, const double* Bov, int 
     const int nb = (v + 15) / 16, nkq = (v + 3) / 4;
     const bool vec2 = (lda % 2 == 0) && (ldb % 2 == 0) && (((uintptr_t)Bvv | (uintptr_t)B) % 16 == 0);
     if (vec2)
-        k_df_gemm<2, true><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(Bvv, lda, B, ldb, M, N, naux, v, nb, nkq, v, (long long)slice_stride, 0, dst);
+        k_df_gemm<2, 1><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(Bvv, lda, B, ldb, M, N, naux, v, nb, nkq, v, (long long)slice_stride, 0, dst, TileSel{{0, 0, 0}});
     else
-        k_df_gemm<1, true><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(Bvv, lda, B, ldb, M, N, naux, v, nb, nkq, v, (long long)slice_stride, 0, dst);
+        k_df_gemm<1, 1><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(Bvv, lda, B, ldb, M, N, naux, v, nb, nkq, v, (long long)slice_stride, 0, dst, TileSel{{0, 0, 0}});
+    return cudaGetLastError();
+}
+
+// abcijk schedule: for every occupied x the part of I_x[d][b][c] = (bd|cx) with b and c in the three tiles (A, B, C) of one tile
+// orbit, in the W-builder's chunk layout over the 3 x 3 local tile pairs (x at dst + x * x_stride).  One GEMM:
+// M = 48 v rows (d, lu, bl), N = 48 o columns (x, lv, cl), K = naux.  Indices at or beyond v come out as zeros.
+cudaError_t tc_launch_df_slices_orbit(const double* Bvv, const double* Bov, int o, int v, int naux, int tA, int tB, int tC, double* dst,
+                                      size_t x_stride, cudaStream_t stream) {
+    const int M = 48 * v, N = 48 * o;
+    const size_t lda = (size_t)v * v, ldb = (size_t)o * v;
+    dim3 grid((N + BN - 1) / BN, (M + BM - 1) / BM);
+    if (grid.y > 65535) return cudaErrorInvalidConfiguration;
+    const int nkq = (v + 3) / 4;
+    const TileSel ts{{tA, tB, tC}};
+    const bool vec2 = (v % 2 == 0) && (((uintptr_t)Bvv | (uintptr_t)Bov) % 16 == 0);
+    if (vec2)
+        k_df_gemm<2, 2><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(Bvv, lda, Bov, ldb, M, N, naux, v, 0, nkq, v, (long long)x_stride, 0, dst, ts);
+    else
+        k_df_gemm<1, 2><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(Bvv, lda, Bov, ldb, M, N, naux, v, 0, nkq, v, (long long)x_stride, 0, dst, ts);
     return cudaGetLastError();
 }
 

@@ -239,7 +239,9 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             if (particle) {
                 const int zp = n >> 1;
                 const size_t nb = (size_t)((v + T - 1) / T);
-                d.b_src = a.slices + (size_t)rec.s[zp] * a.slice_stride + ((size_t)bv[pu] * nb + bv[pvv]) * (size_t)npc * B_STAGE;
+                // tile pair (n1 tile, n2 tile): global tile indices, or (abcijk schedule) their positions in this orbit's (A, B, C)
+                const size_t pair = a.orbit_local ? (size_t)(pu * 3 + pvv) : (size_t)bv[pu] * nb + bv[pvv];
+                d.b_src = a.slices + (size_t)rec.s[zp] * a.slice_stride + pair * (size_t)npc * B_STAGE;
                 d.b_c3 = 0;
             } else {
                 d.b_src = nullptr;

@@ -410,3 +410,38 @@ def test_partitioned_ranges_sum_to_the_full_energy(ctx, world):
     assert covered == n
     assert_energy(sum(parts), E_ref)
     assert abs(sum(parts) - E_full) <= 1e-13 * abs(E_full)
+
+
+# ---- NEXT-2: the paper's abcijk schedule -- tile orbits outer, all triplets inner, integrals rebuilt per tile ----
+@pytest.mark.parametrize("o,v,naux,seed", [(4, 24, 6, 9), (5, 37, 9, 13), (6, 40, 20, 6), (9, 50, 10, 23)])
+def test_abcijk_schedule(ctx, o, v, naux, seed):
+    """Same kernels, the paper's own loop order: E against the oracle, and the per-orbit energies against the oracle's sums
+    restricted to the points of each tile orbit (tco_S_from_W_tile_orbit); a sub-range of orbits sums its own orbits."""
+    p = harness.make_problem(o, v, naux, seed, sigma_B=0.25, blocks=True)
+    dp = DevProblem(p)
+    E_ref, _ = oracle.triples_energy(p)
+    Eorb_ref = oracle.orbit_energies(p, 16)
+    norb = binding_mod.tile_orbit_count(v)
+    assert norb == len(Eorb_ref) == len(oracle.tile_orbits(v, 16))
+    nb = ctx.workspace_bytes_abcijk(o, v, naux)
+    # O(o v T^2) of integrals instead of o v^3: at cfg1 size the footprint is a quarter of the resident schedule's
+    assert ctx.workspace_bytes_abcijk(20, 200, 600) < 0.3 * ctx.workspace_bytes(20, 200, 600)
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    Eorb = torch.full((norb,), float("nan"), dtype=torch.float64, device="cuda")
+    E = ctx.triples_energy_abcijk(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws, workspace_bytes=nb,
+                                  E_orbit_dev=Eorb)
+    st = ctx.get_stats()
+    assert st["kernel"] == TC_KERNEL_TMA and st["n_blocks"] == norb and st["slices_built"] == norb * o
+    assert_energy(E, E_ref)
+    got = Eorb.cpu().numpy()
+    assert np.abs(got - Eorb_ref).max() <= REL_TOL * np.abs(Eorb_ref).max(), (got, Eorb_ref)
+    assert abs(got.sum() - E) <= 1e-12 * abs(E)
+    # a middle range of orbits
+    f0, cnt = norb // 3, max(1, norb // 2)
+    E2 = ctx.triples_energy_abcijk(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws, workspace_bytes=nb,
+                                   orbit_first=f0, orbit_count=cnt, E_orbit_dev=Eorb)
+    assert abs(E2 - Eorb_ref[f0:f0 + cnt].sum()) <= REL_TOL * np.abs(Eorb_ref).max() * cnt
+    assert np.abs(Eorb.cpu().numpy()[:cnt] - Eorb_ref[f0:f0 + cnt]).max() <= REL_TOL * np.abs(Eorb_ref).max()
+    with pytest.raises(binding_mod.TcError):
+        ctx.triples_energy_abcijk(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws, workspace_bytes=nb,
+                                  orbit_first=norb, orbit_count=1)

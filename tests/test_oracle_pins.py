@@ -350,6 +350,36 @@ def test_pair_panels_and_amplitude_rows():
     assert S_rows[0] == pytest.approx(S_full[0], rel=1e-12)
 
 
+def test_tile_orbit_sums_partition_S():
+    """tco_S_from_W_tile_orbit (the per-tile sums of the abcijk scheme): the orbits partition the abc cube, so the restricted sums
+    add up to tco_S_from_W; each one equals a numpy mask over Y R / D built from the oracle's own Y and W."""
+    p = harness.make_problem(3, 7, 5, seed=8, sigma_B=0.3, sigma_t1=0.05, blocks=True)
+    o, v, T = p.o, p.v, 3            # tiles of 3, 3, 1 virtual indices
+    i, j, k = 2, 1, 0
+    W = oracle.W_triplet(o, v, i, j, k, p.t2, p.vvvo[i], p.vvvo[j], p.vvvo[k], p.ovoo)
+    S, Y = oracle.S_from_W(o, v, i, j, k, p.eps_occ, p.eps_vir, p.t1, p.ovov, W, want_Y=True)
+    R = (4 * W + W.transpose(2, 0, 1) + W.transpose(1, 2, 0) - 2 * W.transpose(0, 2, 1) - 2 * W.transpose(2, 1, 0)
+         - 2 * W.transpose(1, 0, 2))      # R[a,b,c] = 4W_abc + W_bca + W_cab - 2W_acb - 2W_cba - 2W_bac
+    ev = p.eps_vir
+    D = p.eps_occ[i] + p.eps_occ[j] + p.eps_occ[k] - ev[:, None, None] - ev[None, :, None] - ev[None, None, :]
+    term = Y * R / D
+    assert term.sum() == pytest.approx(S, rel=1e-13)
+    tile = np.arange(v) // T
+    total = 0.0
+    orbs = oracle.tile_orbits(v, T)
+    assert len(orbs) == 10 and orbs[0] == (0, 0, 0) and orbs[-1] == (2, 2, 2)
+    for (A, B, C) in orbs:
+        got = oracle.S_from_W_tile_orbit(o, v, i, j, k, p.eps_occ, p.eps_vir, p.t1, p.ovov, W, T, A, B, C)
+        key = np.sort(np.stack(np.meshgrid(tile, tile, tile, indexing="ij"), -1), -1)[..., ::-1]
+        mask = (key[..., 0] == A) & (key[..., 1] == B) & (key[..., 2] == C)
+        assert got == pytest.approx(term[mask].sum(), rel=1e-12, abs=1e-18)
+        total += got
+    assert total == pytest.approx(S, rel=1e-13)
+    E_orb = oracle.orbit_energies(p, T)
+    E, _ = oracle.triples_energy(p)
+    assert E_orb.sum() == pytest.approx(E, rel=1e-12)
+
+
 def test_triplet_index_is_a_bijection():
     for o in (1, 2, 5, 9):
         seen = []
