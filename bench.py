@@ -299,6 +299,7 @@ def run_ours(args):
             full_s = ctx.workspace_bytes_streamed(o, v, naux)
             ldv = v + (v % 2)
             nb16, nkq = (v + 15) // 16, (v + 3) // 4
+            nkq += nkq % 2
             per_slot = (nb16 * nb16 * nkq * 8192 + 255) // 256 * 256 + (o * v * ldv * 8 + 255) // 256 * 256
             nb_s = ctx.workspace_bytes_streamed(o, v, naux, full_s - (o - max(3, o // 2)) * per_slot)
             ws_s = ws[:nb_s] if nb_s <= nb else torch.empty(nb_s, dtype=torch.uint8, device="cuda")

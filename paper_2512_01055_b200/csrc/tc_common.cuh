@@ -102,6 +102,13 @@ cudaError_t tc_launch_tile_slice(const double* src, int K, int v, size_t ld, dou
 // (ov|oo)^T[z][x][m][ldo] from the caller's block ovoo[z][x][l][m] (blocks input); the pad column is zeroed
 cudaError_t tc_launch_transpose_ovoo(const double* ovoo, int o, int v, int ldo, double* dst, cudaStream_t stream);
 
+// K chunks (of 4) per tile pair in the tiled slice layout: rounded up to even, so that the steps that consume two K chunks per
+// ring stage (ragged n1 / n2 tiles, tc_wbuild_tma.cu "paired" modes) never read past a tile; the extra chunk is zero padding
+__host__ __device__ inline int tc_tiled_kchunks(int K) {
+    const int n = (K + 3) / 4;
+    return n + (n & 1);
+}
+
 // a3-a6: fused W-builder + epilogue over a list of triplets (tc_wbuild_tma.cu, tc_wbuild.cu).
 // One record per triplet.  The slots say where the per-occupied-index operands of the triplet live: slice slot s[p]
 // holds the (vv|v.) slice of occ[p], amplitude slot t[p] holds the row t2[occ[p]][:][:][:] (slot = index when
@@ -140,7 +147,8 @@ struct tc_wbuild_args {
 };
 // TMA descriptors of the tensor-box operand streams (tc_wbuild_tma.cu); the slices are read with plain bulk copies.
 struct tc_wbuild_maps {
-    CUtensorMap T2h;    // t2 as hole B        [tslot][l][n1][n2]
+    CUtensorMap T2h;    // t2 as hole B        [tslot][l][n1][n2], box of 16 n1 rows
+    CUtensorMap T2h8;   // the same with a box of 8 n1 rows (steps whose n1 tile has at most 8 valid indices)
     CUtensorMap T2p;    // t2 as particle A    [tslot][y][m][d]
     CUtensorMap OvooT;  // (ov|oo)^T as hole A [z][x][m][l]
     bool valid;

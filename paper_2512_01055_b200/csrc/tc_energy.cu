@@ -75,7 +75,7 @@ bool make_layout(int o, int v, int naux, Mode mode, bool bounded, size_t budget,
     if (mode == MODE_ABCIJK) {
         // tile-restricted slices: 3 x 3 local tile pairs instead of nb^2, for all o occupied indices, double buffered
         L->off_ovov = take(sizeof(double) * O * O * V * V);
-        L->slice_stride = align_up(sizeof(double) * 9 * (size_t)((v + 3) / 4) * 1024) / sizeof(double);
+        L->slice_stride = align_up(sizeof(double) * 9 * (size_t)tc_tiled_kchunks(v) * 1024) / sizeof(double);
         L->orbit_buf_stride = O * L->slice_stride;
         L->off_vvvo = take(sizeof(double) * 2 * L->orbit_buf_stride);
         L->off_Eorb = take(sizeof(double) * (size_t)L->n_orbits);

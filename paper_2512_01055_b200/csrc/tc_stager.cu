@@ -225,7 +225,7 @@ cudaError_t tc_launch_df_slices_tiled(const double* Bvv, const double* Bov, int 
     const double* B = Bov + (size_t)x0 * v;
     dim3 grid((N + BN - 1) / BN, (M + BM - 1) / BM);
     if (grid.y > 65535) return cudaErrorInvalidConfiguration;
-    const int nb = (v + 15) / 16, nkq = (v + 3) / 4;
+    const int nb = (v + 15) / 16, nkq = tc_tiled_kchunks(v);
     const bool vec2 = (lda % 2 == 0) && (ldb % 2 == 0) && (((uintptr_t)Bvv | (uintptr_t)B) % 16 == 0);
     if (vec2)
         k_df_gemm<2, 1><<<grid, GTHREADS, sizeof(GemmSmem), stream>>>(Bvv, lda, B, ldb, M, N, naux, v, nb, nkq, v, (long long)slice_stride, 0, dst, TileSel{{0, 0, 0}});
@@ -243,7 +243,7 @@ cudaError_t tc_launch_df_slices_orbit(const double* Bvv, const double* Bov, int 
     const size_t lda = (size_t)v * v, ldb = (size_t)o * v;
     dim3 grid((N + BN - 1) / BN, (M + BM - 1) / BM);
     if (grid.y > 65535) return cudaErrorInvalidConfiguration;
-    const int nkq = (v + 3) / 4;
+    const int nkq = tc_tiled_kchunks(v);
     const TileSel ts{{tA, tB, tC}};
     const bool vec2 = (v % 2 == 0) && (((uintptr_t)Bvv | (uintptr_t)Bov) % 16 == 0);
     if (vec2)
@@ -254,7 +254,7 @@ cudaError_t tc_launch_df_slices_orbit(const double* Bvv, const double* Bov, int 
 }
 
 cudaError_t tc_launch_tile_slice(const double* src, int K, int v, size_t ld, double* dst, cudaStream_t stream) {
-    const int nb = (v + 15) / 16, nkq = (K + 3) / 4;
+    const int nb = (v + 15) / 16, nkq = tc_tiled_kchunks(K);
     const size_t total = (size_t)nb * nb * nkq * 1024;
     const unsigned grid = (unsigned)std::min<size_t>((total + 255) / 256, 148 * 32);
     k_tile_slice<<<grid, 256, 0, stream>>>(src, K, v, ld, nb, nkq, dst);

@@ -45,7 +45,7 @@ constexpr int NCONS = NCONS_WARPS * 32;   // consumer threads
 constexpr int NFLUSH = 128;               // flusher threads (warps 12-15)
 constexpr int NTHREADS = 512;
 constexpr int B_STAGE = 2 * 16 * KC * 8;  // doubles: [z][n1][k][8]
-constexpr int A_STAGE = 4 * 32;           // doubles: four 8-row blocks [m 8][k 4]
+constexpr int A_STAGE = 2 * 4 * 32;       // doubles: [K chunk 0/1][four 8-row blocks [m 8][k 4]]; chunk 1 only in the paired modes
 constexpr int MAX_STEPS = 36;
 constexpr uint32_t B_HALF_BYTES = 16 * KC * 8 * 8;  // 4096
 constexpr uint32_t A_BOX_BYTES = KC * 16 * 8;       // 512
@@ -54,8 +54,17 @@ constexpr int TBUF_COLS = 128;            // 2 consumer warps per lane quarter x
 constexpr int TMEM_COLS = TBUFS * TBUF_COLS;
 constexpr int EPI_SPLIT = 11;             // epilogue: the consumers take la < 11 of their (lb, lc), the flushers la >= 11 of two pairs
 
+// Step modes.  A step whose n2 (or n1) tile has at most 8 valid indices needs only half of the B stage per K chunk; it then packs
+// TWO K chunks into every ring stage, so that a stage still carries 16 DMMAs per warp (a stage with 8 costs almost as much time:
+// the per-stage synchronisation and the ring's depth in time do not shrink with it):
+//   MODE_Z2: n2 ragged -- stage half kk holds the z = 0 half of chunk 2r + kk
+//   MODE_Y2: n1 ragged -- rows 8 kk .. 8 kk + 7 of stage half z hold the rows n1 = 0..7 of chunk 2r + kk
+// Steps whose m tile is ragged cannot do this (their B chunk is full size) and run with 8 DMMAs per stage.
+constexpr int MODE_PLAIN = 0, MODE_Z2 = 1, MODE_Y2 = 2;
+
 struct Step {
-    int nchunks;
+    int nstages;       // ring stages of the step: K chunks, or pairs of K chunks in the paired modes
+    int mode;
     int particle;      // 1: B = slice (bulk copies), A = t2 rows; 0: hole step, B = amplitude row (boxes), A = (ov|oo)^T
     int nxb, ny, nz;   // 8-blocks with at least one index below v: rows, n1, n2 (1 or 2)
     int W0, U0, V0;    // first virtual index of the m, n1 and n2 tiles
@@ -139,10 +148,52 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
     }
 }
 
+// The paired modes: two K chunks per stage.  MODE_Z2: fb[kk][y] from stage half kk, accumulators [..][y][0];
+// MODE_Y2: fb[kk][z] from rows 8 kk.. of stage half z, accumulators [..][0][z].  NO = blocks of the other column index (1 or 2).
+template <int NXB, int MODE, int NO>
+__device__ __forceinline__ void run_step_paired(double (&acc)[4][2][2][2], ConsumerState& cs, int n) {
+    constexpr uint32_t BST = B_STAGE * 8, AST = A_STAGE * 8;
+    for (int r = 0; r < n; r++) {
+        mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
+        const uint32_t pa = cs.bA + cs.stage * AST;
+        const uint32_t pb = cs.bB + cs.stage * BST;
+        double fa[2][2][NXB], fb[2][NO];
+#pragma unroll
+        for (int kk = 0; kk < 2; kk++)
+#pragma unroll
+            for (int h = 0; h < 2; h++)
+#pragma unroll
+                for (int xb = 0; xb < NXB; xb++) fa[kk][h][xb] = lds64(pa + kk * 1024 + (2 * h + xb) * 256);
+#pragma unroll
+        for (int kk = 0; kk < 2; kk++)
+#pragma unroll
+            for (int q = 0; q < NO; q++)
+                fb[kk][q] = lds64(pb + (MODE == MODE_Z2 ? kk * 4096 + q * 2048 : q * 4096 + kk * 2048));
+#pragma unroll
+        for (int kk = 0; kk < 2; kk++)
+#pragma unroll
+            for (int h = 0; h < 2; h++)
+#pragma unroll
+                for (int xb = 0; xb < NXB; xb++)
+#pragma unroll
+                    for (int q = 0; q < NO; q++) {
+                        if (MODE == MODE_Z2) dmma884(acc[2 * h + xb][q][0][0], acc[2 * h + xb][q][0][1], fa[kk][h][xb], fb[kk][q]);
+                        else dmma884(acc[2 * h + xb][0][q][0], acc[2 * h + xb][0][q][1], fa[kk][h][xb], fb[kk][q]);
+                    }
+        __syncwarp();
+        if (cs.lane == 0) mbar_arrive(cs.empty0 + cs.stage * 8);
+        if (++cs.stage == STAGES) {
+            cs.stage = 0;
+            cs.parity ^= 1;
+        }
+    }
+}
+
 // ---- the kernel ------------------------------------------------------------------------------
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __grid_constant__ CUtensorMap mapT2h,
-             const __grid_constant__ CUtensorMap mapT2p, const __grid_constant__ CUtensorMap mapOvooT) {
+             const __grid_constant__ CUtensorMap mapT2h8, const __grid_constant__ CUtensorMap mapT2p,
+             const __grid_constant__ CUtensorMap mapOvooT) {
     extern __shared__ unsigned char smem_raw[];
     Smem& s = *reinterpret_cast<Smem*>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -195,7 +246,11 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             d.nz = (v - d.V0 > 8) ? 2 : 1;
             const bool particle = (n & 1) != 0;
             d.particle = particle ? 1 : 0;
-            d.nchunks = particle ? npc : nhc;
+            d.mode = (d.nz == 1) ? MODE_Z2 : (d.ny == 1 ? MODE_Y2 : MODE_PLAIN);
+            {
+                const int nchunks = particle ? npc : nhc;
+                d.nstages = (d.mode == MODE_PLAIN) ? nchunks : (nchunks + 1) / 2;
+            }
             // the two (slice role zp, family h) terms this step computes in rows 0-15 and 16-31:
             //   family 0 of role zp: (x,y,z) = (occ[xp], occ[yp], occ[zp]),  m -> position xp, n1 -> yp, n2 -> zp
             //   family 1 of role zp: (y,x,z),                                m -> position yp, n1 -> xp, n2 -> zp
@@ -241,7 +296,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 const size_t nb = (size_t)((v + T - 1) / T);
                 // tile pair (n1 tile, n2 tile): global tile indices, or (abcijk schedule) their positions in this orbit's (A, B, C)
                 const size_t pair = a.orbit_local ? (size_t)(pu * 3 + pvv) : (size_t)bv[pu] * nb + bv[pvv];
-                d.b_src = a.slices + (size_t)rec.s[zp] * a.slice_stride + pair * (size_t)npc * B_STAGE;
+                d.b_src = a.slices + (size_t)rec.s[zp] * a.slice_stride + pair * (size_t)tc_tiled_kchunks(v) * B_STAGE;
                 d.b_c3 = 0;
             } else {
                 d.b_src = nullptr;
@@ -376,6 +431,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             const CUtensorMap* m0 = (pw < 2) ? &mapT2h : &mapT2p;
             asm volatile("prefetch.tensormap [%0];" ::"l"(m0) : "memory");
             if (pw >= 2) asm volatile("prefetch.tensormap [%0];" ::"l"(&mapOvooT) : "memory");
+            else asm volatile("prefetch.tensormap [%0];" ::"l"(&mapT2h8) : "memory");
         }
         const uint32_t full0 = smem_u32(&s.full[0]), empty0 = smem_u32(&s.empty[0]);
         const uint32_t dstB = smem_u32(&s.B[0][0]) + pw * B_HALF_BYTES;
@@ -384,28 +440,44 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         uint32_t wrap = 0;  // how many times the ring has wrapped
         for (int st = 0; st < nsteps; st++) {
             const Step& d = s.steps[st];
-            const int n = d.nchunks;
-            const bool particle = d.particle != 0, bulk = d.b_src != nullptr;
-            const uint32_t tx = d.nz * B_HALF_BYTES + 2 * A_BOX_BYTES;
-            const bool active = (pw >= 2) || (pw < d.nz);
-            const char* bsrc = (const char*)d.b_src + (size_t)pw * B_HALF_BYTES;
-            const int c0 = d.V0 + 8 * pw, c2 = d.U0, c3 = d.b_c3;
+            const int n = d.nstages, mode = d.mode;
+            const bool particle = d.particle != 0;
+            // bytes per stage: plain 2 x 4 KB (B) + 2 x 512 B (A); paired modes 8 KB of B either way and two K chunks of A
+            const uint32_t tx = (mode == MODE_PLAIN) ? 2 * B_HALF_BYTES + 2 * A_BOX_BYTES : 2 * B_HALF_BYTES + 4 * A_BOX_BYTES;
+            const char* bsrc = (const char*)d.b_src;
+            const int V0 = d.V0, U0 = d.U0, c3 = d.b_c3;
             const CUtensorMap* amap = particle ? &mapT2p : &mapOvooT;
             const int a2 = d.a_c2[pw & 1], a3 = d.a_c3[pw & 1], aw = d.W0;
             for (int r = 0; r < n; r++) {
-                // every stream waits, active or not: a stream that ran ahead by two ring turns would alias the
-                // barrier's phase parity
+                // every stream waits: a stream that ran ahead by two ring turns would alias the barrier's phase parity
                 if (wrap > 0) mbar_wait(empty0 + stage * 8, (wrap - 1) & 1);
                 if (leader) {
                     const uint32_t full = full0 + stage * 8;
                     if (pw == 0) mbar_expect_tx(full, tx);
-                    if (active) {
-                        if (pw < 2) {
-                            const uint32_t dst = dstB + stage * (B_STAGE * 8);
-                            if (bulk) bulk_load(dst, bsrc + (size_t)r * (B_STAGE * 8), B_HALF_BYTES, full);
-                            else tma_load_4d(dst, &mapT2h, c0, r * KC, c2, c3, full);
+                    if (pw < 2) {
+                        const uint32_t dst = dstB + stage * (B_STAGE * 8);   // stage half pw
+                        if (mode == MODE_PLAIN) {          // column half z = pw of chunk r
+                            if (particle) bulk_load(dst, bsrc + (size_t)r * (B_STAGE * 8) + pw * B_HALF_BYTES, B_HALF_BYTES, full);
+                            else tma_load_4d(dst, &mapT2h, V0 + 8 * pw, r * KC, U0, c3, full);
+                        } else if (mode == MODE_Z2) {      // column half z = 0 of chunk 2r + pw
+                            const int c = 2 * r + pw;
+                            if (particle) bulk_load(dst, bsrc + (size_t)c * (B_STAGE * 8), B_HALF_BYTES, full);
+                            else tma_load_4d(dst, &mapT2h, V0, c * KC, U0, c3, full);
+                        } else {                            // MODE_Y2: rows n1 = 0..7 of column half z = pw, chunks 2r and 2r + 1
+#pragma unroll
+                            for (int kk = 0; kk < 2; kk++) {
+                                const int c = 2 * r + kk;
+                                if (particle) bulk_load(dst + kk * (B_HALF_BYTES / 2), bsrc + (size_t)c * (B_STAGE * 8) + pw * B_HALF_BYTES, B_HALF_BYTES / 2, full);
+                                else tma_load_4d(dst + kk * (B_HALF_BYTES / 2), &mapT2h8, V0 + 8 * pw, c * KC, U0, c3, full);
+                            }
+                        }
+                    } else {
+                        const uint32_t dst = dstA + stage * (A_STAGE * 8);   // rows 16 (pw - 2) ..
+                        if (mode == MODE_PLAIN) {
+                            tma_load_4d(dst, amap, r * KC, aw, a2, a3, full);
                         } else {
-                            tma_load_4d(dstA + stage * (A_STAGE * 8), amap, r * KC, aw, a2, a3, full);
+                            tma_load_4d(dst, amap, 2 * r * KC, aw, a2, a3, full);
+                            tma_load_4d(dst + (A_STAGE / 2) * 8, amap, (2 * r + 1) * KC, aw, a2, a3, full);
                         }
                     }
                 }
@@ -453,19 +525,23 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     const uint32_t tpark = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(warp >> 2) * 64;
     for (int st = 0; st < nsteps; st++) {
         const Step& d = s.steps[st];
-        // dispatch on the ragged-block counts: the loops inside have compile-time trip counts, so the DMMAs carry no
-        // predicates (predicated mma.sync costs a WARPSYNC + NOP each)
-        const int code = (d.nxb - 1) * 4 + (d.ny - 1) * 2 + (d.nz - 1);
-        const int n = d.nchunks;
-        switch (code) {
-            case 7: run_step<2, 2, 2>(acc, cs, n); break;
-            case 6: run_step<2, 2, 1>(acc, cs, n); break;
-            case 5: run_step<2, 1, 2>(acc, cs, n); break;
-            case 4: run_step<2, 1, 1>(acc, cs, n); break;
-            case 3: run_step<1, 2, 2>(acc, cs, n); break;
-            case 2: run_step<1, 2, 1>(acc, cs, n); break;
-            case 1: run_step<1, 1, 2>(acc, cs, n); break;
-            default: run_step<1, 1, 1>(acc, cs, n); break;
+        // dispatch on the mode and the ragged-block counts: the loops inside have compile-time trip counts, so the DMMAs carry
+        // no predicates (predicated mma.sync costs a WARPSYNC + NOP each)
+        const int n = d.nstages;
+        if (d.mode == MODE_PLAIN) {          // ny == nz == 2
+            if (d.nxb == 2) run_step<2, 2, 2>(acc, cs, n);
+            else run_step<1, 2, 2>(acc, cs, n);
+        } else if (d.mode == MODE_Z2) {
+            const int code = (d.nxb - 1) * 2 + (d.ny - 1);
+            switch (code) {
+                case 3: run_step_paired<2, MODE_Z2, 2>(acc, cs, n); break;
+                case 2: run_step_paired<2, MODE_Z2, 1>(acc, cs, n); break;
+                case 1: run_step_paired<1, MODE_Z2, 2>(acc, cs, n); break;
+                default: run_step_paired<1, MODE_Z2, 1>(acc, cs, n); break;
+            }
+        } else {                              // MODE_Y2: ny == 1, nz == 2
+            if (d.nxb == 2) run_step_paired<2, MODE_Y2, 2>(acc, cs, n);
+            else run_step_paired<1, MODE_Y2, 2>(acc, cs, n);
         }
         // ---- park the step's accumulators in tensor memory; the flushers fold them into the W tiles ----
         const int buf = st & (TBUFS - 1);
@@ -517,6 +593,12 @@ cudaError_t tc_wbuild_make_maps(const tc_wbuild_args& a, int n_tslots, tc_wbuild
         const cuuint32_t box[4] = {8, KC, 16, 1};
         ok = ok && tctma::encode4(&out->T2h, a.t2, dim, str, box);
     }
+    {   // the same view with a box of 8 n1 rows (MODE_Y2 hole steps)
+        const cuuint64_t dim[4] = {v, o, v, (cuuint64_t)n_tslots};
+        const cuuint64_t str[3] = {v * ld, ld, (cuuint64_t)a.t2_row_stride};
+        const cuuint32_t box[4] = {8, KC, 8, 1};
+        ok = ok && tctma::encode4(&out->T2h8, a.t2, dim, str, box);
+    }
     {   // t2[tslot][y][m][d] as dims (d, m, y, tslot): particle A, boxes land as [m][k]
         const cuuint64_t dim[4] = {v, v, o, (cuuint64_t)n_tslots};
         const cuuint64_t str[3] = {ld, v * ld, (cuuint64_t)a.t2_row_stride};
@@ -540,11 +622,12 @@ int tc_wbuild_num_orbits(int v) {
 }
 // one slice in the W-builder's layout: [n1 tile][n2 tile][K chunk][z][n1][k][n2 8], zero padded (doubles)
 size_t tc_wbuild_slice_doubles(int v) {
-    const size_t nb = (size_t)((v + T - 1) / T), nkq = (size_t)((v + KC - 1) / KC);
+    const size_t nb = (size_t)((v + T - 1) / T), nkq = (size_t)tc_tiled_kchunks(v);
     return nb * nb * nkq * B_STAGE;
 }
 
 constexpr int kSmemTma = (int)sizeof(Smem) + 128;
+static_assert(kSmemTma <= 232448, "the unit must fit the 227 KB of opt-in shared memory of one SM");
 
 // per device: called by tc_create with the device current (the attribute is per device, not per process)
 cudaError_t tc_wbuild_configure() {
@@ -556,6 +639,6 @@ cudaError_t tc_launch_wbuild(const tc_wbuild_args& a, const tc_wbuild_maps* maps
     const long long nblocks = (long long)a.n_trip * a.n_orbits;
     if (nblocks <= 0) return cudaSuccess;
     if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    k_wbuild_tma<<<(unsigned)nblocks, NTHREADS, kSmemTma, stream>>>(a, orbits, maps->T2h, maps->T2p, maps->OvooT);
+    k_wbuild_tma<<<(unsigned)nblocks, NTHREADS, kSmemTma, stream>>>(a, orbits, maps->T2h, maps->T2h8, maps->T2p, maps->OvooT);
     return cudaGetLastError();
 }

@@ -43,7 +43,8 @@ def read_golden_S(name):
 
 def tiled_slice_bytes(v):
     """Bytes of one (vv|v.) slice slot in the library's workspace: the slice in the W-builder's tiled layout
-    ([n1 tile][n2 tile][K chunk][2][16][4][8] doubles, zero padded), rounded up to 256 (csrc/tc_energy.cu make_layout)."""
+    ([n1 tile][n2 tile][K chunk][2][16][4][8] doubles, zero padded, an even number of K chunks), rounded up to 256 (csrc/tc_energy.cu make_layout)."""
     nb, nkq = (v + 15) // 16, (v + 3) // 4
+    nkq += nkq % 2          # K chunks per tile pair are rounded up to even
     return (nb * nb * nkq * 1024 * 8 + 255) // 256 * 256
 
