@@ -49,9 +49,10 @@ constexpr int A_STAGE = 2 * 4 * 32;       // doubles: [K chunk 0/1][four 8-row b
 constexpr int MAX_STEPS = 36;
 constexpr uint32_t B_HALF_BYTES = 16 * KC * 8 * 8;  // 4096
 constexpr uint32_t A_BOX_BYTES = KC * 16 * 8;       // 512
-constexpr int TBUFS = 4;                  // TMEM parking buffers
-constexpr int TBUF_COLS = 128;            // 2 consumer warps per lane quarter x 64 columns
-constexpr int TMEM_COLS = TBUFS * TBUF_COLS;
+constexpr int TBUF_COLS = 128;            // one parked step: 2 consumer warps per lane quarter x 64 columns
+constexpr int TB_HOLE = 0;                // TMEM buffers 0-2: the three hole steps of the current arrangement
+constexpr int TB_PART = 3;                // TMEM buffer 3: the particle step handed to the flushers
+constexpr int TMEM_COLS = 4 * TBUF_COLS;
 constexpr int EPI_SPLIT = 11;             // epilogue: the consumers take la < 11 of their (lb, lc), the flushers la >= 11 of two pairs
 
 // Step modes.  A step whose n2 (or n1) tile has at most 8 valid indices needs only half of the B stage per K chunk; it then packs
@@ -84,8 +85,8 @@ struct __align__(128) Smem {
     Step steps[MAX_STEPS];
     unsigned long long full[STAGES];
     unsigned long long empty[STAGES];
-    unsigned long long tfull[TBUFS];   // consumers -> flushers: buffer parked
-    unsigned long long tfree[TBUFS];   // flushers -> consumers: buffer read back
+    unsigned long long tfull;          // consumers -> flushers: a particle step is parked
+    unsigned long long tfree;          // flushers -> consumers: it has been read back
     unsigned long long tdone;          // flushers -> consumers: every step is in the W tiles
     unsigned long long kready;         // producers -> epilogue: the (ov|ov) blocks are staged in the operand ring
     double red[NCONS_WARPS + NFLUSH / 32];
@@ -216,8 +217,9 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     const int nhc = (o + KC - 1) / KC;  // chunks of a hole step
     const int npc = (v + KC - 1) / KC;  // chunks of a particle step
 
-    // ---- the step program: thread (q, n) writes step n of arrangement q: n = 2 y' (hole step whose B is the amplitude
-    //      row of occ[2 - y']) or n = 2 zp + 1 (particle step of slice role zp) ----
+    // ---- the step program: thread (q, n) writes step n of arrangement q.  Order H0 H1 P0 H2 P1 P2: hole step Hy (B = the
+    //      amplitude row of occ[2 - y]) computes two 16-row terms that are the hole parts of two particle steps; each particle
+    //      step Pz (slice role z) starts from the parked results of its two hole terms (see the consumers) ----
     if (tid < MAX_STEPS) {
         int sop[6];
         tcw::arrangement_slots(bv, sop);
@@ -244,7 +246,8 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             d.nxb = (v - d.W0 > 8) ? 2 : 1;
             d.ny = (v - d.U0 > 8) ? 2 : 1;
             d.nz = (v - d.V0 > 8) ? 2 : 1;
-            const bool particle = (n & 1) != 0;
+            const bool particle = (n == 2 || n >= 4);
+            const int sub = (n < 2) ? n : (n == 2 ? 0 : (n == 3 ? 2 : n - 3));   // y of a hole step / z of a particle step
             d.particle = particle ? 1 : 0;
             d.mode = (d.nz == 1) ? MODE_Z2 : (d.ny == 1 ? MODE_Y2 : MODE_PLAIN);
             {
@@ -256,13 +259,13 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             //   family 1 of role zp: (y,x,z),                                m -> position yp, n1 -> xp, n2 -> zp
             int zps[2], hs[2];
             if (particle) {
-                zps[0] = zps[1] = n >> 1;
+                zps[0] = zps[1] = sub;
                 hs[0] = 0;
                 hs[1] = 1;
             } else {
                 // hole steps pair the terms that share the amplitude row of B: occ[2]: (0,0),(1,0); occ[1]: (0,1),(2,0);
                 // occ[0]: (1,1),(2,1)
-                const int yy = n >> 1;
+                const int yy = sub;
                 zps[0] = (yy == 2) ? 1 : 0;
                 hs[0] = (yy == 0) ? 0 : 1;
                 zps[1] = (yy == 0) ? 1 : 2;
@@ -292,7 +295,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 }
             }
             if (particle) {
-                const int zp = n >> 1;
+                const int zp = sub;
                 const size_t nb = (size_t)((v + T - 1) / T);
                 // tile pair (n1 tile, n2 tile): global tile indices, or (abcijk schedule) their positions in this orbit's (A, B, C)
                 const size_t pair = a.orbit_local ? (size_t)(pu * 3 + pvv) : (size_t)bv[pu] * nb + bv[pvv];
@@ -308,10 +311,8 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             mbar_init(smem_u32(&s.full[n]), 1);
             mbar_init(smem_u32(&s.empty[n]), NCONS_WARPS);
         }
-        for (int n = 0; n < TBUFS; n++) {
-            mbar_init(smem_u32(&s.tfull[n]), NCONS_WARPS);
-            mbar_init(smem_u32(&s.tfree[n]), NFLUSH / 32);
-        }
+        mbar_init(smem_u32(&s.tfull), NCONS_WARPS);
+        mbar_init(smem_u32(&s.tfree), NFLUSH / 32);
         mbar_init(smem_u32(&s.tdone), NFLUSH / 32);
         mbar_init(smem_u32(&s.kready), 4);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -333,21 +334,20 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         flusher_bar();
         const int fr = lane >> 2, fk = lane & 3;
         const uint32_t tiles0 = smem_u32(&s.tiles[0]);
-        const uint32_t tfull0 = smem_u32(&s.tfull[0]), tfree0 = smem_u32(&s.tfree[0]);
-        const uint32_t tlane = tmem_base + ((uint32_t)(fw * 32) << 16);
-        for (int st = 0; st < nsteps; st++) {
-            const Step& d = s.steps[st];
-            const int buf = st & (TBUFS - 1);
-            const uint32_t use = (uint32_t)(st / TBUFS);
-            mbar_wait(tfull0 + buf * 8, use & 1);
+        const uint32_t tfull0 = smem_u32(&s.tfull), tfree0 = smem_u32(&s.tfree);
+        const uint32_t tlane = tmem_base + ((uint32_t)(fw * 32) << 16) + TB_PART * TBUF_COLS;
+        // only the particle steps are flushed: they start from their hole terms (parked in TMEM by the same threads), so one
+        // flush carries both contractions of a (tile, orientation) pair -- half the shared-memory traffic of flushing every step
+        const int nflush = nsteps / 2;
+        for (int p = 0; p < nflush; p++) {
+            const int arr = p / 3, zp = p - 3 * arr;
+            const Step& d = s.steps[6 * arr + (zp == 0 ? 2 : zp + 3)];
+            mbar_wait(tfull0, p & 1);
             tmem_fence_after();
             // the step's flush parameters, once, in registers
             const int slot0 = d.slot[0], slot1 = d.slot[1];
             const int smv[2] = {d.sm[0], d.sm[1]}, sn1v[2] = {d.sn1[0], d.sn1[1]}, sn2v[2] = {d.sn2[0], d.sn2[1]};
             const bool same = slot0 == slot1;   // repeated tile indices: the halves meet on one tile
-            // the hole sums enter W with a minus sign (eq. (2)): flip the sign bit on the integer pipe -- the FP64 pipe belongs
-            // to the consumers' DMMAs, every FP64 instruction here queues behind them
-            const int sign = d.particle ? 0 : (int)0x80000000;
             // element (m, n1, n2) of half h sits in the thread (fr, fk) of consumer warp cw = n1 & 7 as acc[2h+xb][y][z][e]
             // with m = 8 xb + fr, n1 = cw + 8 y, n2 = 8 z + 2 fk + e
             const int npass = same ? 2 : 1;
@@ -358,11 +358,11 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                     for (int h = 0; h < 2; h++) {
                         if (same && h != pass) continue;
                         double x[16];   // half h of the thread (fr, fk) of consumer warp cw: columns 32 h .. 32 h + 31 of its 64
-                        tmem_load16(tlane + buf * TBUF_COLS + c2 * 64 + h * 32, x);
+                        tmem_load16(tlane + c2 * 64 + h * 32, x);
                         if (c2 == 1 && (same ? pass == 1 : h == 1)) {   // last read of the buffer: the consumers may park into it again
                             tmem_fence_before();
                             __syncwarp();
-                            if (lane == 0) mbar_arrive(tfree0 + buf * 8);
+                            if (lane == 0) mbar_arrive(tfree0);
                         }
                         const uint32_t tile = tiles0 + (uint32_t)(h ? slot1 : slot0) * (TILE * 8);
                         const int sm = smv[h], sn1 = sn1v[h], sn2 = sn2v[h];
@@ -390,11 +390,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
                                 for (int z = 0; z < 2; z++)
 #pragma unroll
-                                    for (int e = 0; e < 2; e++) {
-                                        const double val = x[((xb * 2 + y) * 2 + z) * 2 + e];
-                                        const double sval = __hiloint2double(__double2hiint(val) ^ sign, __double2loint(val));
-                                        sts64(ad[y][z][e], old[y][z][e] + sval);
-                                    }
+                                    for (int e = 0; e < 2; e++) sts64(ad[y][z][e], old[y][z][e] + x[((xb * 2 + y) * 2 + z) * 2 + e]);
                         }
                     }
                 }
@@ -521,10 +517,29 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
             for (int z = 0; z < 2; z++) acc[x][y][z][0] = acc[x][y][z][1] = 0.0;
 
-    const uint32_t tfull0 = opaque(smem_u32(&s.tfull[0])), tfree0 = opaque(smem_u32(&s.tfree[0]));
+    const uint32_t tfull0 = opaque(smem_u32(&s.tfull)), tfree0 = opaque(smem_u32(&s.tfree));
     const uint32_t tpark = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(warp >> 2) * 64;
+    int nparked = 0;   // particle steps handed to the flushers so far
     for (int st = 0; st < nsteps; st++) {
         const Step& d = s.steps[st];
+        const int n6 = st % 6;                       // position in the arrangement: H0 H1 P0 H2 P1 P2
+        const bool particle = d.particle != 0;
+        if (particle) {
+            // ---- start from the hole terms of this particle step's two targets, parked by this thread: rows 0-15 <- term
+            //      (z, family 0), rows 16-31 <- term (z, family 1); hole sums enter W with a minus sign (eq. (2)) ----
+            //        P0: H0 rows 0-15,  H1 rows 0-15      P1: H0 rows 16-31, H2 rows 0-15      P2: H1 rows 16-31, H2 rows 16-31
+            const int z = (n6 == 2) ? 0 : n6 - 3;
+            const int b0 = (z == 2) ? 1 : 0, h0 = (z == 0) ? 0 : 1;
+            const int b1 = (z == 0) ? 1 : 2, h1 = (z == 2) ? 1 : 0;
+            double lo[16], hi[16];
+            tmem_load16(tpark + (TB_HOLE + b0) * TBUF_COLS + h0 * 32, lo);
+            tmem_load16(tpark + (TB_HOLE + b1) * TBUF_COLS + h1 * 32, hi);
+#pragma unroll
+            for (int q = 0; q < 16; q++) {
+                (&acc[0][0][0][0])[q] = -lo[q];
+                (&acc[2][0][0][0])[q] = -hi[q];
+            }
+        }
         // dispatch on the mode and the ragged-block counts: the loops inside have compile-time trip counts, so the DMMAs carry
         // no predicates (predicated mma.sync costs a WARPSYNC + NOP each)
         const int n = d.nstages;
@@ -543,15 +558,21 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             if (d.nxb == 2) run_step_paired<2, MODE_Y2, 2>(acc, cs, n);
             else run_step_paired<1, MODE_Y2, 2>(acc, cs, n);
         }
-        // ---- park the step's accumulators in tensor memory; the flushers fold them into the W tiles ----
-        const int buf = st & (TBUFS - 1);
-        const uint32_t use = (uint32_t)(st / TBUFS);
-        if (use > 0) mbar_wait(tfree0 + buf * 8, (use - 1) & 1);   // the flushers have read the buffer's previous content
-        tmem_fence_after();
-        tmem_store32(tpark + buf * TBUF_COLS, reinterpret_cast<const double(&)[32]>(acc));
-        tmem_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(tfull0 + buf * 8);
+        // ---- park the step's accumulators in tensor memory ----
+        if (!particle) {
+            // a hole step: kept for the two particle steps that start from it (same threads: no hand-over)
+            const int y = (n6 < 2) ? n6 : 2;
+            tmem_store32(tpark + (TB_HOLE + y) * TBUF_COLS, reinterpret_cast<const double(&)[32]>(acc));
+        } else {
+            // a particle step (hole terms included): the flushers fold it into the W tiles
+            if (nparked > 0) mbar_wait(tfree0, (nparked - 1) & 1);   // the flushers have read the previous one
+            tmem_fence_after();
+            tmem_store32(tpark + TB_PART * TBUF_COLS, reinterpret_cast<const double(&)[32]>(acc));
+            tmem_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tfull0);
+            nparked++;
+        }
 #pragma unroll
         for (int x = 0; x < 4; x++)
 #pragma unroll
