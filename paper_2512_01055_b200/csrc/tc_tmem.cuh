@@ -16,12 +16,14 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {  
 __device__ __forceinline__ void tmem_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tmem_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
-// 32 doubles of this thread -> 64 columns at taddr (lane field = this warp's quarter); completes before returning
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// 32 doubles of this thread -> 64 columns at taddr (lane field = this warp's quarter).  The source registers are read at issue;
+// tmem_wait_st() before the data is read back (tcgen05.ld by this thread, or a hand-over to other warps).
 __device__ __forceinline__ void tmem_store32(uint32_t taddr, const double (&x)[32]) {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x64.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32, %33, %34, %35, %36, %37, %38, %39, %40, %41, %42, %43, %44, %45, %46, %47, %48, %49, %50, %51, %52, %53, %54, %55, %56, %57, %58, %59, %60, %61, %62, %63, %64};"
                  ::"r"(taddr), "r"(__double2loint(x[0])), "r"(__double2hiint(x[0])), "r"(__double2loint(x[1])), "r"(__double2hiint(x[1])), "r"(__double2loint(x[2])), "r"(__double2hiint(x[2])), "r"(__double2loint(x[3])), "r"(__double2hiint(x[3])), "r"(__double2loint(x[4])), "r"(__double2hiint(x[4])), "r"(__double2loint(x[5])), "r"(__double2hiint(x[5])), "r"(__double2loint(x[6])), "r"(__double2hiint(x[6])), "r"(__double2loint(x[7])), "r"(__double2hiint(x[7])), "r"(__double2loint(x[8])), "r"(__double2hiint(x[8])), "r"(__double2loint(x[9])), "r"(__double2hiint(x[9])), "r"(__double2loint(x[10])), "r"(__double2hiint(x[10])), "r"(__double2loint(x[11])), "r"(__double2hiint(x[11])), "r"(__double2loint(x[12])), "r"(__double2hiint(x[12])), "r"(__double2loint(x[13])), "r"(__double2hiint(x[13])), "r"(__double2loint(x[14])), "r"(__double2hiint(x[14])), "r"(__double2loint(x[15])), "r"(__double2hiint(x[15])), "r"(__double2loint(x[16])), "r"(__double2hiint(x[16])), "r"(__double2loint(x[17])), "r"(__double2hiint(x[17])), "r"(__double2loint(x[18])), "r"(__double2hiint(x[18])), "r"(__double2loint(x[19])), "r"(__double2hiint(x[19])), "r"(__double2loint(x[20])), "r"(__double2hiint(x[20])), "r"(__double2loint(x[21])), "r"(__double2hiint(x[21])), "r"(__double2loint(x[22])), "r"(__double2hiint(x[22])), "r"(__double2loint(x[23])), "r"(__double2hiint(x[23])), "r"(__double2loint(x[24])), "r"(__double2hiint(x[24])), "r"(__double2loint(x[25])), "r"(__double2hiint(x[25])), "r"(__double2loint(x[26])), "r"(__double2hiint(x[26])), "r"(__double2loint(x[27])), "r"(__double2hiint(x[27])), "r"(__double2loint(x[28])), "r"(__double2hiint(x[28])), "r"(__double2loint(x[29])), "r"(__double2hiint(x[29])), "r"(__double2loint(x[30])), "r"(__double2hiint(x[30])), "r"(__double2loint(x[31])), "r"(__double2hiint(x[31]))
                  : "memory");
-    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 // 64 columns at taddr -> 32 doubles of this thread
 __device__ __forceinline__ void tmem_load32(uint32_t taddr, double (&x)[32]) {

@@ -13,17 +13,22 @@
 // (the hole B operand depends on y only, so the six 16-row hole terms of an arrangement pair up into three 32-row
 // steps).  Hole results enter W with a minus sign (eq. (2)).
 //
+// Six steps per arrangement, in the order H0 H1 P0 H2 P1 P2: each hole term is the hole part of one particle term, so a hole
+// step's accumulators are parked in tensor memory and the particle steps START from them; one flush then carries both
+// contractions of a (tile, orientation) pair.
+//
 // Roles (512 threads, 1 CTA per SM):
-//   warps 0-7   consumers, warp tile 32 x 32: per K chunk of 4  wait full -> 8 conflict-free LDS.64 -> 16 DMMA.8x8x4 ->
-//               release.  At the end of a step the 32 accumulators of each thread are PARKED in tensor memory
-//               (tcgen05.st, one of four 128-column buffers) and the next step starts at once.
+//   warps 0-7   consumers, warp tile 32 x 32: per ring stage  wait full -> 8 conflict-free LDS.64 -> 16 DMMA.8x8x4 -> release.
+//               A stage is one K chunk of 4, or two K chunks when the n1 or n2 tile is ragged and half the B stage would be
+//               idle (MODE_Z2 / MODE_Y2).  At the end of a step the 32 accumulators of each thread are PARKED in tensor memory
+//               (tcgen05.st): a hole step for the particle steps of the same threads, a particle step for the flushers.
 //   warps 8-11  producers, one operand stream each (B columns 0-7 + expect_tx, B columns 8-15, A rows 0-15, A rows 16-31)
 //               into a 3-stage ring.  Particle B comes from slices the stager laid out in fragment order, 4 KB contiguous
 //               per chunk and column half (cp.async.bulk); hole B and both A operands are cp.async.bulk.tensor boxes that
-//               land in the same fragment order.
-//   warps 12-15 flushers: read the parked accumulators back (tcgen05.ld) and add them into the W tiles, permutation in
-//               the address, sign by step kind -- off the consumers' critical path.
-//   After the last step the consumers run the fused epilogue (tcw::orbit_energy).
+//               land in the same fragment order.  At the end they stage the epilogue's (ov|ov) blocks in the ring memory.
+//   warps 12-15 flushers: read the parked particle steps back (tcgen05.ld) and add them into the W tiles, permutation in
+//               the address -- off the consumers' critical path.
+//   After the last step consumers and flushers run the fused epilogue (tcw::orbit_energy).
 // Ragged tiles are zero-filled (TMA out-of-bounds fill, zero padding of the slices); 8-blocks entirely outside v are
 // neither loaded nor multiplied.  CTA order: tile orbit slow, triplet fast (L2 reuse between concurrent CTAs).
 #include <type_traits>
@@ -532,6 +537,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             const int b0 = (z == 2) ? 1 : 0, h0 = (z == 0) ? 0 : 1;
             const int b1 = (z == 0) ? 1 : 2, h1 = (z == 2) ? 1 : 0;
             double lo[16], hi[16];
+            tmem_wait_st();   // the hole steps' parking stores of this thread
             tmem_load16(tpark + (TB_HOLE + b0) * TBUF_COLS + h0 * 32, lo);
             tmem_load16(tpark + (TB_HOLE + b1) * TBUF_COLS + h1 * 32, hi);
 #pragma unroll
@@ -568,6 +574,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             if (nparked > 0) mbar_wait(tfree0, (nparked - 1) & 1);   // the flushers have read the previous one
             tmem_fence_after();
             tmem_store32(tpark + TB_PART * TBUF_COLS, reinterpret_cast<const double(&)[32]>(acc));
+            tmem_wait_st();
             tmem_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tfull0);
