@@ -108,6 +108,9 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_
                  : "memory");
 }
 
+// a[i] for a runtime i without putting the array into local memory
+__device__ __forceinline__ int pick3(const int (&a)[3], int i) { return i == 0 ? a[0] : (i == 1 ? a[1] : a[2]); }
+
 struct ConsumerState {
     int stage;        // ring position of the next chunk to consume
     uint32_t parity;  // its full-barrier parity
@@ -229,25 +232,28 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         int sop[6];
         tcw::arrangement_slots(bv, sop);
         const int q = tid / 6, n = tid - 6 * q;
-        int before = 0, distinct = 0;
+        int before = 0, distinct = 0, sop_pk = 0;   // sop packed four bits each: runtime lookups without a local array
 #pragma unroll
         for (int q2 = 0; q2 < 6; q2++) {
+            sop_pk |= sop[q2] << (4 * q2);
             if (sop[q2] == q2) {
                 distinct++;
                 if (q2 < q) before++;
             }
         }
+        const int t3[3] = {rec.t[0], rec.t[1], rec.t[2]}, s3[3] = {rec.s[0], rec.s[1], rec.s[2]};
         if (tid == 0) {
             s.nsteps = 6 * distinct;
 #pragma unroll
             for (int q2 = 0; q2 < 6; q2++) s.slot_of_perm[q2] = sop[q2];
         }
-        if (sop[q] == q) {
+        if (((sop_pk >> (4 * q)) & 7) == q) {
             const int pw = c_perm[q][0], pu = c_perm[q][1], pvv = c_perm[q][2];  // which of (A,B,C) is the m / n1 / n2 tile
             Step& d = s.steps[6 * before + n];
-            d.W0 = bv[pw] * T;
-            d.U0 = bv[pu] * T;
-            d.V0 = bv[pvv] * T;
+            const int tU = pick3(bv, pu), tV = pick3(bv, pvv);
+            d.W0 = pick3(bv, pw) * T;
+            d.U0 = tU * T;
+            d.V0 = tV * T;
             d.nxb = (v - d.W0 > 8) ? 2 : 1;
             d.ny = (v - d.U0 > 8) ? 2 : 1;
             d.nz = (v - d.V0 > 8) ? 2 : 1;
@@ -286,25 +292,25 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
                 for (int q3 = 0; q3 < 6; q3++)
                     if (c_perm[q3][pm] == pw && c_perm[q3][pn1] == pu && c_perm[q3][pn2] == pvv) qq = q3;
-                d.slot[hh] = sop[qq];
+                d.slot[hh] = (sop_pk >> (4 * qq)) & 7;
                 d.sm[hh] = (pm == 0) ? T * T : (pm == 1 ? T : 0);
                 d.sn1[hh] = (pn1 == 0) ? T * T : (pn1 == 1 ? T : 0);
                 d.sn2[hh] = (pn2 == 0) ? T * T : (pn2 == 1 ? T : 0);
                 if (particle) {   // A = t2[x][y][m][d] (family 0) or t2[y][x][m][d] (family 1): box coordinates (second index, row slot)
-                    d.a_c2[hh] = h ? occ[xp] : occ[yp];
-                    d.a_c3[hh] = h ? rec.t[yp] : rec.t[xp];
+                    d.a_c2[hh] = h ? pick3(occ, xp) : pick3(occ, yp);
+                    d.a_c3[hh] = h ? pick3(t3, yp) : pick3(t3, xp);
                 } else {          // A = (ov|oo)^T[z][x'][m][l], x' = x (family 0) or y (family 1)
-                    d.a_c2[hh] = h ? occ[yp] : occ[xp];
-                    d.a_c3[hh] = occ[zp];
-                    d.b_c3 = h ? rec.t[xp] : rec.t[yp];   // B = t2[y'][l][n1][n2], y' = y (family 0) or x (family 1): the same row for both halves
+                    d.a_c2[hh] = h ? pick3(occ, yp) : pick3(occ, xp);
+                    d.a_c3[hh] = pick3(occ, zp);
+                    d.b_c3 = h ? pick3(t3, xp) : pick3(t3, yp);   // B = t2[y'][l][n1][n2], y' = y (family 0) or x (family 1): the same row for both halves
                 }
             }
             if (particle) {
                 const int zp = sub;
                 const size_t nb = (size_t)((v + T - 1) / T);
                 // tile pair (n1 tile, n2 tile): global tile indices, or (abcijk schedule) their positions in this orbit's (A, B, C)
-                const size_t pair = a.orbit_local ? (size_t)(pu * 3 + pvv) : (size_t)bv[pu] * nb + bv[pvv];
-                d.b_src = a.slices + (size_t)rec.s[zp] * a.slice_stride + pair * (size_t)tc_tiled_kchunks(v) * B_STAGE;
+                const size_t pair = a.orbit_local ? (size_t)(pu * 3 + pvv) : (size_t)tU * nb + tV;
+                d.b_src = a.slices + (size_t)pick3(s3, zp) * a.slice_stride + pair * (size_t)tc_tiled_kchunks(v) * B_STAGE;
                 d.b_c3 = 0;
             } else {
                 d.b_src = nullptr;
