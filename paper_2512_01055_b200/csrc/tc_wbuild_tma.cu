@@ -411,9 +411,9 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         }
         tmem_fence_before();
         flusher_bar();
+        if (lane == 0) mbar_arrive(smem_u32(&s.tdone));   // before the deallocation: nobody waits for that
         if (warp == 12) tmem_dealloc(tmem_base, TMEM_COLS);
         __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&s.tdone));
         // ---- the flushers' share of the fused epilogue: la >= EPI_SPLIT of the pairs ft and ft + 128 ----
         mbar_wait(smem_u32(&s.kready), 0);
         double sum = tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, occ, a, ft, EPI_SPLIT, T) +
