@@ -92,7 +92,8 @@ struct __align__(128) Smem {
     unsigned long long empty[STAGES];
     unsigned long long tfull;          // consumers -> flushers: a particle step is parked
     unsigned long long tfree;          // flushers -> consumers: it has been read back
-    unsigned long long tdone;          // flushers -> consumers: every step is in the W tiles
+    unsigned long long tdone;          // flushers -> consumers: every step but the last is in the W tiles
+    unsigned long long tlast;          // consumers -> flushers: the last step has read its hole terms, tensor memory is idle
     unsigned long long kready;         // producers -> epilogue: the (ov|ov) blocks are staged in the operand ring
     double red[NCONS_WARPS + NFLUSH / 32];
     int slot_of_perm[6];
@@ -325,6 +326,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         mbar_init(smem_u32(&s.tfull), NCONS_WARPS);
         mbar_init(smem_u32(&s.tfree), NFLUSH / 32);
         mbar_init(smem_u32(&s.tdone), NFLUSH / 32);
+        mbar_init(smem_u32(&s.tlast), NCONS_WARPS);
         mbar_init(smem_u32(&s.kready), 4);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -349,7 +351,8 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         const uint32_t tlane = tmem_base + ((uint32_t)(fw * 32) << 16) + TB_PART * TBUF_COLS;
         // only the particle steps are flushed: they start from their hole terms (parked in TMEM by the same threads), so one
         // flush carries both contractions of a (tile, orientation) pair -- half the shared-memory traffic of flushing every step
-        const int nflush = nsteps / 2;
+        // ... except the unit's last step, which the consumers (idle by then) add in from their registers
+        const int nflush = nsteps / 2 - 1;
         for (int p = 0; p < nflush; p++) {
             const int arr = p / 3, zp = p - 3 * arr;
             const Step& d = s.steps[6 * arr + (zp == 0 ? 2 : zp + 3)];
@@ -412,10 +415,15 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         tmem_fence_before();
         flusher_bar();
         if (lane == 0) mbar_arrive(smem_u32(&s.tdone));   // before the deallocation: nobody waits for that
-        if (warp == 12) tmem_dealloc(tmem_base, TMEM_COLS);
+        if (warp == 12) {
+            mbar_wait(smem_u32(&s.tlast), 0);   // the consumers have read the hole terms of the last step: nobody uses tensor memory any more
+            tmem_fence_after();
+            tmem_dealloc(tmem_base, TMEM_COLS);
+        }
         __syncwarp();
         // ---- the flushers' share of the fused epilogue: la >= EPI_SPLIT of the pairs ft and ft + 128 ----
         mbar_wait(smem_u32(&s.kready), 0);
+        asm volatile("bar.sync 4, %0;" ::"n"(NCONS + NFLUSH) : "memory");   // the consumers have added the last step in
         double sum = tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, occ, a, ft, EPI_SPLIT, T) +
                      tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, occ, a, ft + NFLUSH, EPI_SPLIT, T);
 #pragma unroll
@@ -500,7 +508,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             const uint32_t fills = wrap + (q < stage ? 1u : 0u);
             if (fills > 0) mbar_wait(empty0 + q * 8, (fills - 1) & 1);
         }
-        tcw::stage_panels(&s.B[0][0], bv, occ, a, tid - NCONS, 128);
+        tcw::stage_panels(&s.B[0][0], bv, occ, a, tid - NCONS);
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&s.kready));
         return;
@@ -551,6 +559,11 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 (&acc[0][0][0][0])[q] = -lo[q];
                 (&acc[2][0][0][0])[q] = -hi[q];
             }
+            if (st == nsteps - 1) {   // this warp's last access to tensor memory: the flushers may deallocate it
+                tmem_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&s.tlast));
+            }
         }
         // dispatch on the mode and the ragged-block counts: the loops inside have compile-time trip counts, so the DMMAs carry
         // no predicates (predicated mma.sync costs a WARPSYNC + NOP each)
@@ -575,6 +588,44 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             // a hole step: kept for the two particle steps that start from it (same threads: no hand-over)
             const int y = (n6 < 2) ? n6 : 2;
             tmem_store32(tpark + (TB_HOLE + y) * TBUF_COLS, reinterpret_cast<const double(&)[32]>(acc));
+        } else if (st == nsteps - 1) {
+            // ---- the unit's last step: nothing is left to multiply, so the consumers add it into the W tiles themselves,
+            //      straight from the registers (256 threads, no round trip through tensor memory) ----
+            mbar_wait(smem_u32(&s.tdone), 0);   // every earlier step is in the tiles
+            const int fr = lane >> 2, fk = lane & 3;
+            const uint32_t tiles0 = smem_u32(&s.tiles[0]);
+            const bool same = d.slot[0] == d.slot[1];
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                if (h == 1 && same) consumer_bar();   // the halves meet on one tile: one after the other
+                const uint32_t tile = tiles0 + (uint32_t)d.slot[h] * (TILE * 8);
+                const int sm = d.sm[h], sn1 = d.sn1[h], sn2 = d.sn2[h];
+                // element acc[2h+xb][y][z][e] = (m, n1, n2) = (8 xb + fr, warp + 8 y, 8 z + 2 fk + e), as in the flushers
+                const int lin0 = fr * sm + warp * sn1 + 2 * fk * sn2;
+                const int rot0 = fr + warp + 2 * fk;
+#pragma unroll
+                for (int xb = 0; xb < 2; xb++) {
+                    uint32_t ad[2][2][2];
+                    double old[2][2][2];
+#pragma unroll
+                    for (int y = 0; y < 2; y++)
+#pragma unroll
+                        for (int z = 0; z < 2; z++)
+#pragma unroll
+                            for (int e = 0; e < 2; e++) {
+                                const int lin = lin0 + 8 * xb * sm + 8 * y * sn1 + (8 * z + e) * sn2;
+                                const int rot = (rot0 + 8 * xb + 8 * y + 8 * z + e) & (T - 1);
+                                ad[y][z][e] = tile + (uint32_t)(lin + rot) * 8;
+                                old[y][z][e] = lds64(ad[y][z][e]);
+                            }
+#pragma unroll
+                    for (int y = 0; y < 2; y++)
+#pragma unroll
+                        for (int z = 0; z < 2; z++)
+#pragma unroll
+                            for (int e = 0; e < 2; e++) sts64(ad[y][z][e], old[y][z][e] + acc[2 * h + xb][y][z][e]);
+                }
+            }
         } else {
             // a particle step (hole terms included): the flushers fold it into the W tiles
             if (nparked > 0) mbar_wait(tfree0, (nparked - 1) & 1);   // the flushers have read the previous one
@@ -593,9 +644,8 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
                 for (int z = 0; z < 2; z++) acc[x][y][z][0] = acc[x][y][z][1] = 0.0;
     }
-    mbar_wait(smem_u32(&s.tdone), 0);   // every step has been added into the W tiles
-    mbar_wait(smem_u32(&s.kready), 0);  // and the epilogue's (ov|ov) blocks are staged
-    consumer_bar();
+    mbar_wait(smem_u32(&s.kready), 0);  // the epilogue's (ov|ov) blocks are staged
+    asm volatile("bar.sync 4, %0;" ::"n"(NCONS + NFLUSH) : "memory");   // every step is in the W tiles (consumers + flushers)
 
     if (a.W_debug) tcw::dump_W(s.tiles, s.slot_of_perm, bv, v, a.W_debug, tid, NCONS);
     double sum = tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, occ, a, tid, 0, EPI_SPLIT);
