@@ -204,8 +204,10 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __grid_constant__ CUtensorMap mapT2h,
              const __grid_constant__ CUtensorMap mapT2h8, const __grid_constant__ CUtensorMap mapT2p,
              const __grid_constant__ CUtensorMap mapOvooT) {
-    extern __shared__ unsigned char smem_raw[];
-    Smem& s = *reinterpret_cast<Smem*>(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    // no integer round trip in this cast: the compiler then knows that everything reached through `s` is shared memory (LDS / STS
+    // with 32-bit addresses instead of generic loads)
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    Smem& s = *reinterpret_cast<Smem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int o = a.o, v = a.v;
 
@@ -710,7 +712,7 @@ size_t tc_wbuild_slice_doubles(int v) {
     return nb * nb * nkq * B_STAGE;
 }
 
-constexpr int kSmemTma = (int)sizeof(Smem) + 128;
+constexpr int kSmemTma = (int)sizeof(Smem);
 static_assert(kSmemTma <= 232448, "the unit must fit the 227 KB of opt-in shared memory of one SM");
 
 // per device: called by tc_create with the device current (the attribute is per device, not per process)
