@@ -140,6 +140,10 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
         for (int y = 0; y < NY; y++)
 #pragma unroll
             for (int z = 0; z < NZ; z++) fb[y][z] = lds64(pb + z * 4096 + y * 2048);
+        // the chunk's fragments are in registers: hand the stage back before multiplying (the arrive is a release: the loads
+        // above are performed before the producers can see it), which gives the refill a head start of one chunk of DMMAs
+        __syncwarp();
+        if (cs.lane == 0) mbar_arrive(cs.empty0 + cs.stage * 8);
 #pragma unroll
         for (int h = 0; h < 2; h++)
 #pragma unroll
@@ -148,9 +152,6 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
                 for (int y = 0; y < NY; y++)
 #pragma unroll
                     for (int z = 0; z < NZ; z++) dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[h][xb], fb[y][z]);
-        // every DMMA that reads this chunk's fragments has been issued (operands are read at issue): hand the stage back
-        __syncwarp();
-        if (cs.lane == 0) mbar_arrive(cs.empty0 + cs.stage * 8);
         if (++cs.stage == STAGES) {
             cs.stage = 0;
             cs.parity ^= 1;
@@ -179,6 +180,8 @@ __device__ __forceinline__ void run_step_paired(double (&acc)[4][2][2][2], Consu
 #pragma unroll
             for (int q = 0; q < NO; q++)
                 fb[kk][q] = lds64(pb + (MODE == MODE_Z2 ? kk * 4096 + q * 2048 : q * 4096 + kk * 2048));
+        __syncwarp();
+        if (cs.lane == 0) mbar_arrive(cs.empty0 + cs.stage * 8);
 #pragma unroll
         for (int kk = 0; kk < 2; kk++)
 #pragma unroll
@@ -190,8 +193,6 @@ __device__ __forceinline__ void run_step_paired(double (&acc)[4][2][2][2], Consu
                         if (MODE == MODE_Z2) dmma884(acc[2 * h + xb][q][0][0], acc[2 * h + xb][q][0][1], fa[kk][h][xb], fb[kk][q]);
                         else dmma884(acc[2 * h + xb][0][q][0], acc[2 * h + xb][0][q][1], fa[kk][h][xb], fb[kk][q]);
                     }
-        __syncwarp();
-        if (cs.lane == 0) mbar_arrive(cs.empty0 + cs.stage * 8);
         if (++cs.stage == STAGES) {
             cs.stage = 0;
             cs.parity ^= 1;
@@ -424,10 +425,11 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
         }
         __syncwarp();
         // ---- the flushers' share of the fused epilogue: la >= EPI_SPLIT of the pairs ft and ft + 128 ----
+        const tcw::EpiBC pre0 = tcw::epilogue_prefetch(bv, occ, a, ft), pre1 = tcw::epilogue_prefetch(bv, occ, a, ft + NFLUSH);
         mbar_wait(smem_u32(&s.kready), 0);
         asm volatile("bar.sync 4, %0;" ::"n"(NCONS + NFLUSH) : "memory");   // the consumers have added the last step in
-        double sum = tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, occ, a, ft, EPI_SPLIT, T) +
-                     tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, occ, a, ft + NFLUSH, EPI_SPLIT, T);
+        double sum = tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, a, pre0, ft, EPI_SPLIT, T) +
+                     tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, a, pre1, ft + NFLUSH, EPI_SPLIT, T);
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
         if (lane == 0) s.red[NCONS_WARPS + fw] = sum;
@@ -646,11 +648,12 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
 #pragma unroll
                 for (int z = 0; z < 2; z++) acc[x][y][z][0] = acc[x][y][z][1] = 0.0;
     }
+    const tcw::EpiBC pre = tcw::epilogue_prefetch(bv, occ, a, tid);   // in flight across the two waits below
     mbar_wait(smem_u32(&s.kready), 0);  // the epilogue's (ov|ov) blocks are staged
     asm volatile("bar.sync 4, %0;" ::"n"(NCONS + NFLUSH) : "memory");   // every step is in the W tiles (consumers + flushers)
 
     if (a.W_debug) tcw::dump_W(s.tiles, s.slot_of_perm, bv, v, a.W_debug, tid, NCONS);
-    double sum = tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, occ, a, tid, 0, EPI_SPLIT);
+    double sum = tcw::orbit_energy(s.tiles, &s.B[0][0], s.slot_of_perm, bv, a, pre, tid, 0, EPI_SPLIT);
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
     if (lane == 0) s.red[warp] = sum;
