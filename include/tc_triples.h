@@ -161,6 +161,26 @@ tc_status tc_triples_energy_slice(tc_ctx* ctx, int o, int v,
                                   void* stream, long long first, long long count,
                                   double* S_dev, double* E_partial_out);
 
+/* The same with NO allocation anywhere on its path, for callers that cannot allocate (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the scratch the kernels use (what `workspace` is above) lives in
+ * one file-scope device array of TC_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads the library holds
+ * until the process exits.  The caller passes only inputs and outputs (arguments as in tc_triples_energy_slice).
+ *   Limit: the problem must fit the array with everything resident, i.e. tc_workspace_bytes(ctx, o, v, naux_or_0, 0) <=
+ *   TC_STATIC_SCRATCH_BYTES (e.g. (o,v,naux) = (8,40,120), (6,72,24), (10,48,150)); beyond that TC_ERR_WORKSPACE_TOO_SMALL with
+ *   the two sizes in tc_last_error, and nothing is launched.
+ *   Sharing: all calls on a device use the same array and find the last call's contents in it.  The call clears the part it
+ *   uses first (stream ordered), so a result never depends on an earlier call; calls that OVERLAP on one GPU (different
+ *   streams or threads) race on the array: serialise them.
+ *   Calls no cudaMalloc / cudaFree / allocating library routine; synchronises `stream` once to return the host double, like
+ *   the other energy calls. */
+#define TC_STATIC_SCRATCH_BYTES (64u << 20)
+tc_status tc_triples_energy_static(tc_ctx* ctx, int o, int v,
+                                   const double* eps_occ, const double* eps_vir,
+                                   const double* t1, const double* t2,
+                                   const tc_int_blocks* blocks, const tc_df_factors* df,
+                                   void* stream, long long first, long long count,
+                                   double* S_dev, double* E_partial_out);
+
 /* Host-resident amplitudes (the paper streams t2 pieces with cudaMemcpyAsync under the integral
  * build, Fig. 2 l.6, 9: at o=150, v=1150 the amplitudes are 238 GB).  As
  * tc_triples_energy_slice with DF input, except that `t2_host` is HOST memory (pinned for the copies to

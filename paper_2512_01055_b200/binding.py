@@ -51,11 +51,13 @@ class TcStats(ctypes.Structure):
         return {name: getattr(self, name) for name, _ in self._fields_}
 
 
+STATIC_SCRATCH_BYTES = 64 << 20   # TC_STATIC_SCRATCH_BYTES of include/tc_triples.h
+
 EXPORTS = [
     "tc_create", "tc_destroy", "tc_status_string", "tc_last_error",
     "tc_triplet_count", "tc_triplet_decode", "tc_triplet_index", "tc_triplet_partition",
     "tc_workspace_bytes", "tc_workspace_bytes_streamed", "tc_plan_summary", "tc_plan_dump", "tc_build_blocks",
-    "tc_triples_energy", "tc_triples_energy_slice", "tc_triples_energy_streamed", "tc_triples_energy_host",
+    "tc_triples_energy", "tc_triples_energy_slice", "tc_triples_energy_static", "tc_triples_energy_streamed", "tc_triples_energy_host",
     "tc_tile_orbit_count", "tc_workspace_bytes_abcijk", "tc_triples_energy_abcijk",
     "tc_debug_W_triplet",
     "tc_get_stats", "tc_bench_dmma_peak", "tc_bench_dfma_peak", "tc_bench_copy_bw", "tc_bench_ring_peak",
@@ -101,6 +103,7 @@ def lib() -> ctypes.CDLL:
     L.tc_triples_energy.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_IntBlocks), _P(_DfFactors), _vp, _sz, _vp, _P(_d)]
     L.tc_triples_energy_slice.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_IntBlocks), _P(_DfFactors), _vp, _sz, _vp,
                                           _ll, _ll, _vp, _P(_d)]
+    L.tc_triples_energy_static.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _P(_IntBlocks), _P(_DfFactors), _vp, _ll, _ll, _vp, _P(_d)]
     L.tc_triples_energy_host.argtypes = [_vp, _i, _i, _i] + [_vp] * 7 + [_ll, _ll, _P(_d), _P(_sz)]
     L.tc_debug_W_triplet.argtypes = [_vp, _i, _i, _i, _i, _i, _vp, _P(_IntBlocks), _vp, _vp]
     L.tc_get_stats.argtypes = [_vp, _P(TcStats)]
@@ -202,6 +205,15 @@ class Context:
         self._check(lib().tc_triples_energy_slice(self._h, o, v, _ptr(eps_occ), _ptr(eps_vir), _ptr(t1), _ptr(t2), pb, pd,
                                                   _ptr(workspace), workspace_bytes, _stream(stream), first, count,
                                                   _ptr(S_dev), ctypes.byref(E)))
+        return E.value
+
+    def triples_energy_static(self, o, v, eps_occ, eps_vir, t1, t2, *, blocks=None, df=None, stream=None, first=0, count=0,
+                              S_dev=None) -> float:
+        """As triples_energy_slice, with the scratch in the library's static device array (STATIC_SCRATCH_BYTES): no allocation."""
+        b, d, pb, pd = self._ints(blocks, df)
+        E = _d()
+        self._check(lib().tc_triples_energy_static(self._h, o, v, _ptr(eps_occ), _ptr(eps_vir), _ptr(t1), _ptr(t2), pb, pd,
+                                                   _stream(stream), first, count, _ptr(S_dev), ctypes.byref(E)))
         return E.value
 
     def triples_energy_streamed(self, o, v, eps_occ, eps_vir, t1, t2_host, *, df, workspace, workspace_bytes, stream=None,
