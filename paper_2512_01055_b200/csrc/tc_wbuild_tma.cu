@@ -556,12 +556,11 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             const int b1 = (z == 0) ? 1 : 2, h1 = (z == 2) ? 1 : 0;
             double lo[16], hi[16];
             tmem_wait_st();   // the hole steps' parking stores of this thread
-            tmem_load16(tpark + (TB_HOLE + b0) * TBUF_COLS + h0 * 32, lo);
-            tmem_load16(tpark + (TB_HOLE + b1) * TBUF_COLS + h1 * 32, hi);
+            tmem_load16_neg_pair(tpark + (TB_HOLE + b0) * TBUF_COLS + h0 * 32, tpark + (TB_HOLE + b1) * TBUF_COLS + h1 * 32, lo, hi);
 #pragma unroll
             for (int q = 0; q < 16; q++) {
-                (&acc[0][0][0][0])[q] = -lo[q];
-                (&acc[2][0][0][0])[q] = -hi[q];
+                (&acc[0][0][0][0])[q] = lo[q];
+                (&acc[2][0][0][0])[q] = hi[q];
             }
             if (st == nsteps - 1) {   // this warp's last access to tensor memory: the flushers may deallocate it
                 tmem_fence_before();
