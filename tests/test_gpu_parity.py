@@ -445,3 +445,52 @@ def test_abcijk_schedule(ctx, o, v, naux, seed):
     with pytest.raises(binding_mod.TcError):
         ctx.triples_energy_abcijk(o, v, dp.eps_occ, dp.eps_vir, dp.t1, dp.t2, df=dp.df(), workspace=ws, workspace_bytes=nb,
                                   orbit_first=norb, orbit_count=1)
+
+
+# ---- stream semantics: "work is enqueued on `stream`; the side stream is forked and joined with events so the caller sees
+#      single-stream semantics" (include/tc_triples.h) --------------------------------------------------------------------------
+@pytest.mark.parametrize("regime", ["resident", "blocked", "abcijk", "static"])
+def test_caller_stream_ordering(ctx, regime):
+    """Every input is PRODUCED on a non-blocking caller stream right before the call (behind ~10 ms of other work on that
+    stream), and holds NaN until then: a library that ran on another stream, or whose side stream did not wait for the fork
+    event, would read the NaNs.  The result must equal the default-stream result to the bit."""
+    p = harness.make_problem(9, 24, 10, 41, sigma_B=0.25, blocks=False)
+    dp = DevProblem(p)
+    o, v, naux = p.o, p.v, p.naux
+    n = oracle.triplet_count(o)
+    names = ("eps_occ", "eps_vir", "t1", "t2", "Boo", "Bov", "Bvv")
+    if regime == "blocked":
+        nb = ctx.workspace_bytes(o, v, naux, ctx.workspace_bytes(o, v, naux) - (o - 3) * harness.tiled_slice_bytes(v))
+    elif regime == "abcijk":
+        nb = ctx.workspace_bytes_abcijk(o, v, naux)
+    else:
+        nb = ctx.workspace_bytes(o, v, naux)
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+
+    def call(t, stream):
+        df = (naux, t["Boo"], t["Bov"], t["Bvv"])
+        S = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
+        a = (o, v, t["eps_occ"], t["eps_vir"], t["t1"], t["t2"])
+        if regime == "abcijk":
+            return ctx.triples_energy_abcijk(*a, df=df, workspace=ws, workspace_bytes=nb, stream=stream), None
+        if regime == "static":
+            return ctx.triples_energy_static(*a, df=df, stream=stream, first=0, count=n, S_dev=S), S
+        return ctx.triples_energy_slice(*a, df=df, workspace=ws, workspace_bytes=nb, stream=stream, first=0, count=n, S_dev=S), S
+
+    ref = {k: getattr(dp, k) for k in names}
+    E_ref, S_ref = call(ref, None)
+    if regime == "blocked":
+        assert ctx.get_stats()["n_blocks"] >= 2
+    late = {k: torch.full_like(ref[k], float("nan")) for k in names}
+    junk = torch.randn(4096, 4096, device="cuda")
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()                          # non-blocking: no implicit ordering with the legacy default stream
+    with torch.cuda.stream(s):
+        for _ in range(8):
+            junk = junk @ junk * 1e-3                # keeps the stream busy while the host runs ahead
+        for k in names:
+            late[k].copy_(ref[k])
+        E, S = call(late, s)
+    assert E == E_ref, (regime, E, E_ref)
+    if S is not None:
+        assert (S.cpu().numpy() == S_ref.cpu().numpy()).all()
