@@ -135,8 +135,9 @@ struct tc_wbuild_args {
     const double* slices;            // slot s at slices + s * slice_stride, in the W-builder's tiled layout
                                      // [n1 tile][n2 tile][K chunk][z][n1 16][k 4][n2 8], zero padded (tc_wbuild_slice_doubles)
     size_t slice_stride;             // doubles
-    int orbit_local;                 // 1 (abcijk schedule): the slices hold only the 3 x 3 tile pairs of the launch's one tile orbit,
+    int orbit_local;                 // 1 (abcijk schedule): the slices hold only the 3 x 3 tile pairs of each tile orbit of the launch,
                                      // pair (lu, lv) = positions of the n1 / n2 tile in (A, B, C)
+    size_t orbit_stride;             // orbit_local: doubles between the slice sets of consecutive orbits of the launch
     const double* ovooT;             // [z][x][m][ldo] = (l z | x m): the (ov|oo) block with the contracted index fastest
     const double* ovov;              // [j][k][b][c] (natural layout; read by the epilogue only)
     const tc_trip_rec* recs;         // device array [n_trip]
@@ -174,8 +175,8 @@ cudaError_t tc_launch_make_triplets(int o, long long first, int n, tc_trip_rec* 
 //   S[dest ? dest[t] : t] = sum_u partial[t][u], fixed order
 cudaError_t tc_launch_reduce_units(const double* partial, int n_trip, int n_units, const int* dest, double* S, cudaStream_t stream);
 //   abcijk schedule: S[t] = (first ? 0 : S[t]) + partial[t];  *E_orbit = sum_t w[t] * partial[t] (fixed order, one block)
-cudaError_t tc_launch_accumulate_orbit(const double* partial, const double* w, long long n, int first, double* S, double* E_orbit,
-                                       cudaStream_t stream);
+cudaError_t tc_launch_accumulate_orbit(const double* partial, int stride, const double* w, long long n, int first, double* S,
+                                       double* E_orbit, cudaStream_t stream);
 //   *E = sum_t w[t] * S[t], fixed order, one block
 cudaError_t tc_launch_reduce_energy(const double* S, const double* w, long long n, double* E, cudaStream_t stream);
 

@@ -36,7 +36,13 @@ struct Layout {
     size_t orbit_buf_stride;   // abcijk schedule: doubles between the two staging buffers (o tile-restricted slices each)
 };
 
+#ifndef TC_ORBIT_GROUP
+#define TC_ORBIT_GROUP 2
+#endif
 constexpr size_t kPartialBudget = (size_t)256 << 20;
+// abcijk schedule: tile orbits per W-builder launch.  One orbit is N_trip equal units, i.e. N_trip / 148 waves with a ragged last
+// one (cfg1: 10.3 -> 11); two orbits of different length per launch smooth that out for one more staging buffer set.
+constexpr int kOrbitGroup = TC_ORBIT_GROUP;
 
 // bounded == false: size for everything resident (tc_workspace_bytes with hbm_budget 0).
 bool make_layout(int o, int v, int naux, Mode mode, bool bounded, size_t budget, Layout* L) {
@@ -77,7 +83,7 @@ bool make_layout(int o, int v, int naux, Mode mode, bool bounded, size_t budget,
         L->off_ovov = take(sizeof(double) * O * O * V * V);
         L->slice_stride = align_up(sizeof(double) * 9 * (size_t)tc_tiled_kchunks(v) * 1024) / sizeof(double);
         L->orbit_buf_stride = O * L->slice_stride;
-        L->off_vvvo = take(sizeof(double) * 2 * L->orbit_buf_stride);
+        L->off_vvvo = take(sizeof(double) * 2 * kOrbitGroup * L->orbit_buf_stride);   // two sets (double buffering) of kOrbitGroup orbits
         L->off_Eorb = take(sizeof(double) * (size_t)L->n_orbits);
     } else if (mode == MODE_BLOCKS) {
         L->off_vvvo = take(sizeof(double) * O * L->slice_stride);
@@ -507,7 +513,9 @@ extern "C" tc_status tc_triples_energy_abcijk(tc_ctx* ctx, int o, int v, const d
     if (orbit_first < 0 || orbit_count < 0 || orbit_first + orbit_count > L.n_orbits)
         TC_FAIL(ctx, TC_ERR_INVALID_ARG, "orbit range [%lld,%lld) outside [0,%d)", orbit_first, orbit_first + orbit_count, L.n_orbits);
     const long long ntrip = tc_triplet_count(o);
-    if ((long long)L.batch * L.n_orbits < ntrip || ntrip > 0x7fffffffLL) TC_FAIL(ctx, TC_ERR_INTERNAL, "partial buffer too small for %lld triplets", ntrip);
+    const int group = std::min(kOrbitGroup, L.n_orbits);
+    if ((long long)L.batch * L.n_orbits < ntrip * group || ntrip * group > 0x7fffffffLL)
+        TC_FAIL(ctx, TC_ERR_INTERNAL, "partial buffer too small for %lld triplets x %d orbits", ntrip, group);
     TC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t s = (cudaStream_t)stream, side = ctx->side_stream;
     char* ws = (char*)workspace;
@@ -533,7 +541,7 @@ extern "C" tc_status tc_triples_energy_abcijk(tc_ctx* ctx, int o, int v, const d
     if (L.ldo != o) TC_CUDA(ctx, cudaMemsetAsync(w_ovooT, 0, sizeof(double) * O * O * V * (size_t)L.ldo, s));
     TC_CUDA(ctx, launch_ovooT(df, o, v, L.ldo, w_ovooT, s));
     TC_CUDA(ctx, launch_ovov(df, o, v, w_ovov, s));
-    TC_CUDA(ctx, cudaMemsetAsync(w_buf, 0, sizeof(double) * 2 * L.orbit_buf_stride, s));   // K padding of the chunk layout stays zero
+    TC_CUDA(ctx, cudaMemsetAsync(w_buf, 0, sizeof(double) * 2 * kOrbitGroup * L.orbit_buf_stride, s));   // K padding of the chunk layout stays zero
     TC_CUDA(ctx, tc_launch_make_triplets(o, 0, (int)ntrip, d_recs, d_w, s));
     ctx->stats.n_kernel_launches += 3;
     tc_wbuild_args a;
@@ -549,6 +557,7 @@ extern "C" tc_status tc_triples_energy_abcijk(tc_ctx* ctx, int o, int v, const d
     a.ovov = w_ovov;
     a.slice_stride = L.slice_stride;
     a.orbit_local = 1;
+    a.orbit_stride = L.orbit_buf_stride;
     a.recs = d_recs;
     a.n_trip = (int)ntrip;
     a.partial = d_partial;
@@ -571,27 +580,35 @@ extern "C" tc_status tc_triples_energy_abcijk(tc_ctx* ctx, int o, int v, const d
     TC_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
     TimingRing kring(ctx->ev_k0, ctx->ev_k1), gring(ctx->ev_g0, ctx->ev_g1);
     TC_CUDA(ctx, cudaEventRecord(ctx->ev_c0, s));
-    for (long long n = 0; n < orbit_count; n++) {
-        const int4 ob = orb[(size_t)(orbit_first + n)];
-        double* buf = w_buf + (size_t)(n & 1) * L.orbit_buf_stride;
-        // staging buffer n & 1 was last read by orbit n - 2
-        if (n >= 2) TC_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_done[(n - 2) % TC_EV_RING], 0));
+    long long ngroups = 0;
+    for (long long n = 0; n < orbit_count; n += group, ngroups++) {
+        const long long q = ngroups;                      // launch number
+        const int g_n = (int)std::min<long long>(group, orbit_count - n);
+        double* buf = w_buf + (size_t)(q & 1) * kOrbitGroup * L.orbit_buf_stride;
+        // staging buffer set q & 1 was last read by launch q - 2
+        if (q >= 2) TC_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_done[(q - 2) % TC_EV_RING], 0));
         const int g = gring.next();
         TC_CUDA(ctx, cudaEventRecord(ctx->ev_g0[g], side));
-        TC_CUDA(ctx, tc_launch_df_slices_orbit(df->Bvv, df->Bov, o, v, df->naux, ob.x, ob.y, ob.z, buf, L.slice_stride, side));
+        for (int m = 0; m < g_n; m++) {
+            const int4 ob = orb[(size_t)(orbit_first + n + m)];
+            TC_CUDA(ctx, tc_launch_df_slices_orbit(df->Bvv, df->Bov, o, v, df->naux, ob.x, ob.y, ob.z, buf + (size_t)m * L.orbit_buf_stride,
+                                                   L.slice_stride, side));
+        }
         TC_CUDA(ctx, cudaEventRecord(ctx->ev_g1[g], side));
-        TC_CUDA(ctx, cudaEventRecord(ctx->ev_staged[n % TC_EV_RING], side));
-        TC_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_staged[n % TC_EV_RING], 0));
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_staged[q % TC_EV_RING], side));
+        TC_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_staged[q % TC_EV_RING], 0));
         const int kslot = kring.next();
         TC_CUDA(ctx, cudaEventRecord(ctx->ev_k0[kslot], s));
         a.slices = buf;
+        a.n_orbits = g_n;                                 // partial sums of the launch: [triplet][g_n]
         TC_CUDA(ctx, tc_launch_wbuild(a, &maps, d_orbits + (orbit_first + n), s));
         TC_CUDA(ctx, cudaEventRecord(ctx->ev_k1[kslot], s));
-        TC_CUDA(ctx, tc_launch_accumulate_orbit(d_partial, d_w, ntrip, n == 0 ? 1 : 0, d_S, d_Eorb + n, s));
-        TC_CUDA(ctx, cudaEventRecord(ctx->ev_done[n % TC_EV_RING], s));
-        ctx->stats.n_kernel_launches += 3;
-        ctx->stats.n_work_units += ntrip;
-        ctx->stats.slices_built += o;
+        for (int m = 0; m < g_n; m++)                     // orbit by orbit, in order: S and the per-orbit energies do not depend on the grouping
+            TC_CUDA(ctx, tc_launch_accumulate_orbit(d_partial + m, g_n, d_w, ntrip, (n + m) == 0 ? 1 : 0, d_S, d_Eorb + n + m, s));
+        TC_CUDA(ctx, cudaEventRecord(ctx->ev_done[q % TC_EV_RING], s));
+        ctx->stats.n_kernel_launches += 1 + 2 * g_n;
+        ctx->stats.n_work_units += ntrip * g_n;
+        ctx->stats.slices_built += (long long)o * g_n;
     }
     ctx->stats.n_blocks = orbit_count;
     TC_CUDA(ctx, cudaEventRecord(ctx->ev_c1, s));

@@ -81,12 +81,13 @@ __global__ void __launch_bounds__(1024) k_reduce_energy(const double* __restrict
 }
 
 // abcijk schedule: fold one tile orbit's per-triplet partials into S and form the orbit's partial energy
-__global__ void __launch_bounds__(1024) k_accumulate_orbit(const double* __restrict__ partial, const double* __restrict__ w, long long n,
-                                                           int first, double* __restrict__ S, double* __restrict__ E_orbit) {
+// (partial[t * stride]: the launch's partial sums are [triplet][orbit of the launch])
+__global__ void __launch_bounds__(1024) k_accumulate_orbit(const double* __restrict__ partial, int stride, const double* __restrict__ w,
+                                                           long long n, int first, double* __restrict__ S, double* __restrict__ E_orbit) {
     __shared__ double sh[1024];
     double x = 0.0, comp = 0.0;
     for (long long t = threadIdx.x; t < n; t += 1024) {
-        const double p = partial[t];
+        const double p = partial[t * stride];
         S[t] = first ? p : S[t] + p;
         const double y = w[t] * p - comp;
         const double z = x + y;
@@ -99,9 +100,9 @@ __global__ void __launch_bounds__(1024) k_accumulate_orbit(const double* __restr
 
 }  // namespace
 
-cudaError_t tc_launch_accumulate_orbit(const double* partial, const double* w, long long n, int first, double* S, double* E_orbit,
-                                       cudaStream_t stream) {
-    k_accumulate_orbit<<<1, 1024, 0, stream>>>(partial, w, n, first, S, E_orbit);
+cudaError_t tc_launch_accumulate_orbit(const double* partial, int stride, const double* w, long long n, int first, double* S,
+                                       double* E_orbit, cudaStream_t stream) {
+    k_accumulate_orbit<<<1, 1024, 0, stream>>>(partial, stride, w, n, first, S, E_orbit);
     return cudaGetLastError();
 }
 

@@ -118,7 +118,30 @@ struct ConsumerState {
     int lane;
     uint32_t full0, empty0;  // shared addresses of full[0] / empty[0]
     uint32_t bB, bA;         // this thread's fragment addresses in stage 0
+    uint32_t zero;           // 0, but not to the compiler (see release_stage)
 };
+
+// Hands a ring stage back to the producers.  The stage may be refilled as soon as every fragment of it is in registers, but
+// "after the loads in program order" does not say that: a shared-memory load delivers its data asynchronously, and an mbarrier
+// arrive issued behind it can become visible first (observed: with the arrive right behind the loads, about one unit in 20 000
+// multiplied a fragment of the NEXT chunk when the refill was fast; tests/test_gpu_parity.py::test_abcijk_is_bit_reproducible).
+// A DMMA reads its operands at issue and cannot issue before they have landed, so the arrive's address is made to depend on
+// the results of DMMAs that between them take every fragment of the stage as an operand (`bits`, ANDed with a zero the compiler
+// cannot see): wherever the assembler schedules the arrive, and in whatever order it issues the DMMAs, the loads have landed.
+__device__ __forceinline__ uint32_t hi_bits(double x) { return (uint32_t)__double2hiint(x); }
+__device__ __forceinline__ void release_stage(const ConsumerState& cs, uint32_t bits) {
+    const uint32_t bar = cs.empty0 + cs.stage * 8 + (bits & cs.zero);
+    __syncwarp();
+    // lane 0 arrives; predicated, so that the address arithmetic stays outside a divergent branch
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.eq.u32 p, %1, 0;\n"
+        "@p mbarrier.arrive.shared::cta.b64 _, [%0];\n"
+        "}\n" ::"r"(bar),
+        "r"(cs.lane)
+        : "memory");
+}
 
 // One step of the consumer warps: n chunks of  wait full -> LDS -> DMMA -> release.
 // NXB / NY / NZ = number of 8-blocks of rows (per half) / n1 / n2 that reach below v.
@@ -140,10 +163,6 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
         for (int y = 0; y < NY; y++)
 #pragma unroll
             for (int z = 0; z < NZ; z++) fb[y][z] = lds64(pb + z * 4096 + y * 2048);
-        // the chunk's fragments are in registers: hand the stage back before multiplying (the arrive is a release: the loads
-        // above are performed before the producers can see it), which gives the refill a head start of one chunk of DMMAs
-        __syncwarp();
-        if (cs.lane == 0) mbar_arrive(cs.empty0 + cs.stage * 8);
 #pragma unroll
         for (int h = 0; h < 2; h++)
 #pragma unroll
@@ -152,6 +171,17 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
                 for (int y = 0; y < NY; y++)
 #pragma unroll
                     for (int z = 0; z < NZ; z++) dmma884(acc[2 * h + xb][y][z][0], acc[2 * h + xb][y][z][1], fa[h][xb], fb[y][z]);
+        {
+            // a covering set: block (i, i mod nb) resp. (i mod na, i) takes row fragment i and column fragment i mod nb as operands
+            constexpr int NA = 2 * NXB, NB = NY * NZ, NC = NA > NB ? NA : NB;
+            uint32_t bits = 0;
+#pragma unroll
+            for (int i = 0; i < NC; i++) {
+                const int ia = i % NA, ib = i % NB;
+                bits |= hi_bits(acc[2 * (ia / NXB) + ia % NXB][ib / NZ][ib % NZ][0]);
+            }
+            release_stage(cs, bits);
+        }
         if (++cs.stage == STAGES) {
             cs.stage = 0;
             cs.parity ^= 1;
@@ -180,8 +210,6 @@ __device__ __forceinline__ void run_step_paired(double (&acc)[4][2][2][2], Consu
 #pragma unroll
             for (int q = 0; q < NO; q++)
                 fb[kk][q] = lds64(pb + (MODE == MODE_Z2 ? kk * 4096 + q * 2048 : q * 4096 + kk * 2048));
-        __syncwarp();
-        if (cs.lane == 0) mbar_arrive(cs.empty0 + cs.stage * 8);
 #pragma unroll
         for (int kk = 0; kk < 2; kk++)
 #pragma unroll
@@ -193,6 +221,18 @@ __device__ __forceinline__ void run_step_paired(double (&acc)[4][2][2][2], Consu
                         if (MODE == MODE_Z2) dmma884(acc[2 * h + xb][q][0][0], acc[2 * h + xb][q][0][1], fa[kk][h][xb], fb[kk][q]);
                         else dmma884(acc[2 * h + xb][0][q][0], acc[2 * h + xb][0][q][1], fa[kk][h][xb], fb[kk][q]);
                     }
+        {
+            // every accumulator block is written by the K chunk kk = 1 last, after kk = 0 (a true dependency through the block):
+            // a covering set of blocks therefore covers the fragments of both chunks
+            constexpr int NA = 2 * NXB, NC = NA > NO ? NA : NO;
+            uint32_t bits = 0;
+#pragma unroll
+            for (int i = 0; i < NC; i++) {
+                const int ia = i % NA, q = i % NO;
+                bits |= hi_bits(MODE == MODE_Z2 ? acc[2 * (ia / NXB) + ia % NXB][q][0][0] : acc[2 * (ia / NXB) + ia % NXB][0][q][0]);
+            }
+            release_stage(cs, bits);
+        }
         if (++cs.stage == STAGES) {
             cs.stage = 0;
             cs.parity ^= 1;
@@ -314,7 +354,8 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 const size_t nb = (size_t)((v + T - 1) / T);
                 // tile pair (n1 tile, n2 tile): global tile indices, or (abcijk schedule) their positions in this orbit's (A, B, C)
                 const size_t pair = a.orbit_local ? (size_t)(pu * 3 + pvv) : (size_t)tU * nb + tV;
-                d.b_src = a.slices + (size_t)pick3(s3, zp) * a.slice_stride + pair * (size_t)tc_tiled_kchunks(v) * B_STAGE;
+                d.b_src = a.slices + (a.orbit_local ? (size_t)orbit * a.orbit_stride : 0) + (size_t)pick3(s3, zp) * a.slice_stride +
+                          pair * (size_t)tc_tiled_kchunks(v) * B_STAGE;
                 d.b_c3 = 0;
             } else {
                 d.b_src = nullptr;
@@ -524,6 +565,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
     cs.stage = 0;
     cs.parity = 0;
     cs.lane = lane;
+    cs.zero = (uint32_t)a.n_trip >> 31;   // 0 (n_trip is positive); a kernel argument, so not foldable
     cs.full0 = opaque(smem_u32(&s.full[0]));
     cs.empty0 = opaque(smem_u32(&s.empty[0]));
     {

@@ -115,3 +115,20 @@ def test_cfg4_sampled_against_golden(ctx):
     triplets run through the blocked schedule with side-stream staging."""
     st = _check_sampled(ctx, "cfg4", halo=2)
     assert st["n_blocks"] >= 1 and st["slices_built"] >= 3
+
+
+def test_abcijk_is_bit_reproducible(ctx):
+    """100 launches of one tile orbit x all 1540 triplets of cfg1 (the abcijk schedule's launch shape: every operand of the
+    launch fits L2, so the ring is refilled as fast as it ever is), on two orbits that contain the ragged tile 12 (paired-K
+    stages: the most fragment loads per stage).  A ring stage handed back before its fragment loads have landed shows up here as
+    a different energy in a few per cent of the launches (csrc/tc_wbuild_tma.cu, release_stage)."""
+    p, d = _device_problem("cfg1")
+    nb = ctx.workspace_bytes_abcijk(p.o, p.v, p.naux)
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    for orbit in (409, 427):     # tiles (12, 9, 0) and (12, 10, 8)
+        seen = set()
+        for _ in range(100):
+            seen.add(ctx.triples_energy_abcijk(p.o, p.v, d["eps_occ"], d["eps_vir"], d["t1"], d["t2"],
+                                               df=(p.naux, d["Boo"], d["Bov"], d["Bvv"]), workspace=ws, workspace_bytes=nb,
+                                               orbit_first=orbit, orbit_count=1))
+        assert len(seen) == 1, (orbit, sorted(seen))

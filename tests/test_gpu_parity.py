@@ -424,7 +424,7 @@ def test_abcijk_schedule(ctx, o, v, naux, seed):
     norb = binding_mod.tile_orbit_count(v)
     assert norb == len(Eorb_ref) == len(oracle.tile_orbits(v, 16))
     nb = ctx.workspace_bytes_abcijk(o, v, naux)
-    # O(o v T^2) of integrals instead of o v^3: at cfg1 size the footprint is a quarter of the resident schedule's
+    # O(o v T^2) of integrals instead of o v^3: at cfg1 size the footprint is under a third of the resident schedule's (two tile orbits per launch)
     assert ctx.workspace_bytes_abcijk(20, 200, 600) < 0.3 * ctx.workspace_bytes(20, 200, 600)
     ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
     Eorb = torch.full((norb,), float("nan"), dtype=torch.float64, device="cuda")
