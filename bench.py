@@ -366,9 +366,9 @@ def run_ours(args):
     if world == 1 and not args.no_configs and args.config == "cfg1":
         del ws
         configs = {}
-        plan = [("cfg2", 5000, 296), ("cfg3", 20000, 100), ("h2o14", 30000, 592), ("20,201,600,1", 0, 1540)]
+        plan = [("cfg2", 5000, 296), ("cfg3", 20000, 300), ("h2o14", 30000, 592), ("20,201,600,1", 0, 1540)]
         if torch.cuda.mem_get_info()[1] > 170e9:
-            plan.append(("cfg4", 59640, 48))
+            plan.append(("cfg4", 59640, 96))
         for name, f0, cnt in plan:
             try:
                 configs[name] = measure_slice(ctx, torch, synth, name, f0, cnt, dmma_sus)
