@@ -292,7 +292,11 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             for (int q2 = 0; q2 < 6; q2++) s.slot_of_perm[q2] = sop[q2];
         }
         if (((sop_pk >> (4 * q)) & 7) == q) {
-            const int pw = c_perm[q][0], pu = c_perm[q][1], pvv = c_perm[q][2];  // which of (A,B,C) is the m / n1 / n2 tile
+            // c_perm and its inverse packed into constants: lookups with runtime indices by shifts instead of dependent
+            // constant-memory loads (the step table is on every unit's critical path)
+            constexpr unsigned long long PERM_PK = tcw::perm_packed();
+            constexpr unsigned int PERM_INV = tcw::perm_inverse_packed();
+            const int pw = (int)(PERM_PK >> (6 * q)) & 3, pu = (int)(PERM_PK >> (6 * q + 2)) & 3, pvv = (int)(PERM_PK >> (6 * q + 4)) & 3;  // which of (A,B,C) is the m / n1 / n2 tile
             Step& d = s.steps[6 * before + n];
             const int tU = pick3(bv, pu), tV = pick3(bv, pvv);
             d.W0 = pick3(bv, pw) * T;
@@ -332,10 +336,9 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
                 const int xp = (zp == 0) ? 1 : 0;
                 const int yp = (zp == 2) ? 1 : 2;
                 const int pm = h ? yp : xp, pn1 = h ? xp : yp, pn2 = zp;
-                int qq = 0;
-#pragma unroll
-                for (int q3 = 0; q3 < 6; q3++)
-                    if (c_perm[q3][pm] == pw && c_perm[q3][pn1] == pu && c_perm[q3][pn2] == pvv) qq = q3;
+                // the ordering that has tile role pw at position pm, pu at pn1, pvv at pn2
+                const int a0 = (pm == 0) ? pw : (pn1 == 0 ? pu : pvv), a1 = (pm == 1) ? pw : (pn1 == 1 ? pu : pvv);
+                const int qq = (int)(PERM_INV >> (3 * (4 * a0 + a1))) & 7;
                 d.slot[hh] = (sop_pk >> (4 * qq)) & 7;
                 d.sm[hh] = (pm == 0) ? T * T : (pm == 1 ? T : 0);
                 d.sn1[hh] = (pn1 == 0) ? T * T : (pn1 == 1 ? T : 0);
@@ -362,7 +365,7 @@ k_wbuild_tma(const tc_wbuild_args a, const int4* __restrict__ orbits, const __gr
             }
         }
     }
-    if (tid == 0) {
+    if (tid == 2 * 32) {   // a warp that builds no step: in parallel with the table
         for (int n = 0; n < STAGES; n++) {
             mbar_init(smem_u32(&s.full[n]), 1);
             mbar_init(smem_u32(&s.empty[n]), NCONS_WARPS);
