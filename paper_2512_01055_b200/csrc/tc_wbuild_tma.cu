@@ -68,6 +68,8 @@ constexpr int EPI_SPLIT = 11;             // epilogue: the consumers take la < 1
 // Steps whose m tile is ragged cannot do this (their B chunk is full size) and run with 8 DMMAs per stage.
 constexpr int MODE_PLAIN = 0, MODE_Z2 = 1, MODE_Y2 = 2;
 
+// (104 bytes: an odd number of 8-byte words.  The 36 table-building threads write their records at this stride; 112- or
+// 128-byte records measured 1.5 % slower.)
 struct Step {
     int nstages;       // ring stages of the step: K chunks, or pairs of K chunks in the paired modes
     int mode;
@@ -81,6 +83,7 @@ struct Step {
     int sm[2], sn1[2], sn2[2];  // address strides of m, n1, n2 in that tile (0 for the rotated last coordinate)
 };
 
+static_assert(sizeof(Step) == 104, "see the comment at Step");
 static_assert(STAGES * (B_STAGE + A_STAGE) >= tcw::KST_DOUBLES, "the epilogue stages its (ov|ov) blocks in the operand ring");
 
 struct __align__(128) Smem {
