@@ -153,6 +153,7 @@ __device__ __forceinline__ void release_stage(const ConsumerState& cs, uint32_t 
 template <int NXB, int NY, int NZ>
 __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerState& cs, int n) {
     constexpr uint32_t BST = B_STAGE * 8, AST = A_STAGE * 8;  // stage strides in bytes
+#pragma unroll 2   // measured: +0.3 % over the rolled loop, 3 and 4 no better
     for (int r = 0; r < n; r++) {
         mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
         const uint32_t pa = cs.bA + cs.stage * AST;
@@ -197,6 +198,7 @@ __device__ __forceinline__ void run_step(double (&acc)[4][2][2][2], ConsumerStat
 template <int NXB, int MODE, int NO>
 __device__ __forceinline__ void run_step_paired(double (&acc)[4][2][2][2], ConsumerState& cs, int n) {
     constexpr uint32_t BST = B_STAGE * 8, AST = A_STAGE * 8;
+#pragma unroll 2   // measured: +0.3 % over the rolled loop, 3 and 4 no better
     for (int r = 0; r < n; r++) {
         mbar_wait(cs.full0 + cs.stage * 8, cs.parity);
         const uint32_t pa = cs.bA + cs.stage * AST;
