@@ -199,8 +199,8 @@ tc_status tc_triples_energy_streamed(tc_ctx* ctx, int o, int v,
 /* The paper's own loop order (the abcijk scheme; Fig. 1; Fig. 2): virtual tile
  * orbits {A >= B >= C} (tile edge 16) outer, all triplets i >= j >= k inner.  For each orbit the (vv|vo) integrals are
  * rebuilt from the DF factors restricted to the orbit's tiles (Fig. 2 l.7, 10), so the footprint beside t2 and (ov|ov) is
- * O(o v 16^2) instead of o v^3; the next orbit's integrals are assembled on the library's side stream while the current
- * orbit's contraction runs.  Same kernels, same result as tc_triples_energy: E = sum over orbits of the orbit's energy
+ * O(o v 16^2) instead of o v^3; a launch takes two orbits (all triplets x each), and the next launch's integrals are
+ * assembled on the library's side stream while the current one's contraction runs (two sets of staging buffers).  Same kernels, same result as tc_triples_energy: E = sum over orbits of the orbit's energy
  *   E_orbit = sum_{i>=j>=k} (2 - d_ij - d_jk) sum_{(a,b,c) in orbit} (W + Vd) R / D.
  * Orbits orbit_first .. orbit_first+orbit_count-1 of the enumeration A >= B >= C (A slowest) are computed;
  * E_orbit_dev (device, [orbit_count], optional) receives their energies, E_out (host) their sum.  DF input only;
